@@ -1,0 +1,229 @@
+"""Pins of the oracle's scalar pieces against what the paper prints and what mathematics fixes.
+
+Each test compares oracle/ output with something that is NOT the oracle: a value the paper
+prints (tests/golden/paper_pins.json, cited), a closed form / asymptotic limit from the cited
+literature, an independent root finder, or an identity.
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.optimize import brentq
+
+import oracle as orc
+
+GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "paper_pins.json")))
+
+
+# ---------------------------------------------------------------------------------- S0 mass grid
+@pytest.mark.parametrize("g", GOLD["mass_ratio"]["grids"])
+def test_mass_ratio_prints_as_paper(g):
+    """both published grids have m_{n+1}/m_n = 1.38.  N bins <-> N+1 log-spaced
+    EDGES gives 1.3835 / 1.3805; spacing N centres over the range instead would give 1.3880 for
+    the first grid, which prints 1.39 -- so this pins the edge/centre construction."""
+    grid = orc.mass_grid(g["n_bins"], g["a_min_cm"], g["a_max_cm"], 1.6)
+    q = grid.m_c[1:] / grid.m_c[:-1]
+    assert np.allclose(q, q[0], rtol=1e-12)
+    assert f"{q[0]:.2f}" == GOLD["mass_ratio"]["printed"]
+    bins_per_decade = 1.0 / math.log10(q[0])
+    assert bins_per_decade > GOLD["bins_per_decade"]["min"]
+    # alternative construction (centres span the range) must NOT print 1.38 for grid 1
+    if g["n_bins"] == 100:
+        q_alt = (g["a_max_cm"] / g["a_min_cm"]) ** (3.0 / (g["n_bins"] - 1))
+        assert f"{q_alt:.2f}" != GOLD["mass_ratio"]["printed"]
+
+
+def test_mass_grid_geometry():
+    g = orc.mass_grid(40, 1e-5, 1.0, 1.67)
+    assert g.a_e[0] == pytest.approx(1e-5, rel=1e-15) and g.a_e[-1] == pytest.approx(1.0, rel=1e-14)
+    # m = 4 pi/3 rho_m a^3 (solid sphere), centres inside their own edges, geometric means
+    assert np.allclose(g.m_e, 4.0 * math.pi / 3.0 * 1.67 * g.a_e ** 3, rtol=1e-15)
+    assert np.all(g.m_c > g.m_e[:-1]) and np.all(g.m_c < g.m_e[1:])
+    assert np.allclose(g.m_c ** 2, g.m_e[:-1] * g.m_e[1:], rtol=1e-14)
+    assert np.allclose(g.m_c, 4.0 * math.pi / 3.0 * 1.67 * g.a_c ** 3, rtol=1e-13)
+
+
+# ---------------------------------------------------------------------------------- Eq. 62
+def test_pfrag_closed_form_and_limits():
+    assert orc.pfrag(100.0, 100.0) == pytest.approx(GOLD["pfrag_at_vfrag"]["value"], rel=1e-15)
+    assert orc.pfrag(37.0, 37.0) == pytest.approx(GOLD["pfrag_at_vfrag"]["value"], rel=1e-15)
+    assert orc.pfrag(100.0, 1e-3) == 0.0                 # dv -> 0: no fragmentation
+    assert orc.pfrag(100.0, 0.0) == 0.0
+    assert orc.pfrag(100.0, 1e9) == pytest.approx(1.0, abs=1e-12)   # dv -> inf: always fragments
+    # monotone in dv, within [0, 1]  (p_coag = 1 - p_frag must be a probability, Eq. 55)
+    dv = np.logspace(-2, 6, 400)
+    p = np.array([orc.pfrag(100.0, v) for v in dv])
+    assert np.all(np.diff(p) >= -3e-16) and p.min() >= 0 and p.max() <= 1   # monotone to rounding
+    # small-x expansion: 1 - p = x^2/2 - x^3/3 + ..., x = 1.5 (vf/dv)^2
+    x = 1.5 * (100.0 / 1e4) ** 2
+    assert 1.0 - orc.pfrag(100.0, 1e4) == pytest.approx(x * x / 2 - x ** 3 / 3, rel=1e-3)
+
+
+# ---------------------------------------------------------------------------------- St*
+def _ystar_eq(y, St):
+    return (2.0 / 3.0) * y * (y - 1.0) ** 2 - 1.0 / (1.0 + y) + St / (1.0 + St)
+
+
+def test_ystar_matches_independent_root_finder():
+    """The fixed 6-iteration Newton of the oracle against scipy's bracketing root finder on the
+    same equation (Ormel & Cuzzi 2007 Eq. 21d as read in DESIGN.md R4)."""
+    for St in np.concatenate([[0.0, 1e-12, 1e-6], np.linspace(0.001, 1.0, 60)]):
+        y_ref = brentq(_ystar_eq, 0.9, 2.0, args=(St,), xtol=1e-15, rtol=1e-15)
+        assert orc.ystar(St) == pytest.approx(y_ref, rel=2e-15)
+    assert orc.ystar(1.0) == pytest.approx(1.0, abs=1e-15)       # continuous with St >= 1 branch
+    assert orc.ystar(0.0) == pytest.approx(1.6, abs=2e-3)        # OC07's y_a ~ 1.6 for St << 1
+
+
+def test_ststar_bounds_and_monotone():
+    """St* in [Re^-1/2, 1]; monotone non-decreasing in St."""
+    St_eta = 1e-4
+    St = np.logspace(-9, 3, 300)
+    s = np.array([orc.ststar(x, St_eta) for x in St])
+    assert s.min() == St_eta and s.max() == 1.0
+    assert np.all(np.diff(s) >= 0)
+    assert orc.ststar(5.0, St_eta) == 1.0
+    assert orc.ststar(1e-7, St_eta) == St_eta
+
+
+def test_quadratic_fit_claim():
+    """a quadratic fit of St* is 'accurate to within 2%'.  A least-squares quadratic in
+    St to the exact root y*(St) on [0, 1] is good to ~2.0%: corroborates the equation read in R4."""
+    St = np.linspace(0.0, 1.0, 2001)
+    y = np.array([orc.ystar(x) for x in St])
+    c = np.polyfit(St, y, 2)
+    rel = np.abs(np.polyval(c, St) / y - 1.0).max()
+    assert rel < GOLD["ststar_fit_accuracy"]["max_rel_error"] * 1.05
+    assert rel > 0.005          # and it is not trivially exact: the claim is informative
+
+
+# ---------------------------------------------------------------------------------- turbulence
+def _turb(St1, St2, St_eta):
+    S = orc.ststar(St1, St_eta)
+    return orc.vrel2_turb(St1, St2, S, St_eta)
+
+
+def test_turbulent_regime_limits():
+    """Closed-form limits of Ormel & Cuzzi (2007) section 3.4 (their Eqs. 26-29)."""
+    Re = 1e8
+    St_eta = Re ** -0.5
+    # tightly coupled, St << Re^-1/2:  dV^2 = Re^1/2 (St1 - St2)^2   (their Eq. 27)
+    St1, St2 = 1e-7, 0.5e-7
+    assert _turb(St1, St2, St_eta) == pytest.approx(Re ** 0.5 * (St1 - St2) ** 2, rel=2e-2)
+    # equal tightly-coupled grains: exactly no relative velocity
+    assert _turb(1e-7, 1e-7, St_eta) == 0.0
+    # intermediate, Re^-1/2 << St << 1 (their Eq. 28): dV^2 = [2 ya - (1+e) + 2/(1+e)(1/(1+ya) + e^3/(ya+e))] St1
+    ya = orc.ystar(0.0)
+    St1 = 1e-2
+    for e in (1e-3, 0.5, 1.0):
+        expect = (2 * ya - (1 + e) + 2.0 / (1 + e) * (1.0 / (1 + ya) + e ** 3 / (ya + e))) * St1
+        assert _turb(St1, e * St1, 1e-9) == pytest.approx(expect, rel=2e-2)
+    # commonly quoted: ~3 St1 for very unequal grains, ~2 St1 for equal grains
+    assert _turb(1e-3, 1e-9, 1e-12) / 1e-3 == pytest.approx(3.0, rel=2e-2)
+    assert _turb(1e-3, 1e-3, 1e-12) / 1e-3 == pytest.approx(2.0, rel=3e-2)
+    # heavy, St >> 1 (their Eq. 29): dV^2 = 1/(1+St1) + 1/(1+St2)
+    for St1, St2 in ((50.0, 20.0), (1e3, 1e3), (200.0, 3.0)):
+        assert _turb(St1, St2, St_eta) == pytest.approx(1.0 / (1 + St1) + 1.0 / (1 + St2), rel=1e-6)
+
+
+def test_turbulent_velocity_symmetric_entry_and_nonneg():
+    rng = np.random.default_rng(1)
+    for _ in range(300):
+        St1 = 10 ** rng.uniform(-8, 3)
+        St2 = St1 * 10 ** rng.uniform(-6, 0)
+        v = _turb(St1, St2, 10 ** rng.uniform(-6, -2))
+        assert v >= 0.0 and math.isfinite(v)
+
+
+# ---------------------------------------------------------------------------------- full kernel
+def _cell(N=24, T=80.0, rho_g=1e-12, Omega=2e-9, alpha=1e-3, vfrag=100.0, seed=0, vscale=10.0):
+    g = orc.mass_grid(N, 1e-5, 1.0, 1.67)
+    rng = np.random.default_rng(seed)
+    vR = vscale * rng.standard_normal(N)
+    vZ = vscale * rng.standard_normal(N)
+    p = orc.Params(v_frag=vfrag)
+    return g, T, rho_g, Omega, alpha, vR, vZ, p
+
+
+def test_kernel_symmetric_and_brownian_limit():
+    """alpha -> 0 and no laminar motion leaves only Brownian motion (Eq. 58):
+    K_ij = pi (a_i+a_j)^2 sqrt(8 kT (m_i+m_j)/(pi m_i m_j)); equal masses: sqrt(16 kT/(pi m))."""
+    g, T, rho_g, Omega, _, vR, vZ, p = _cell()
+    K, pf, St, Ss = orc.cell_kernel(g, T, rho_g, Omega, 1e-300, 0 * vR, 0 * vZ, p)
+    assert np.array_equal(K, K.T) and np.array_equal(pf, pf.T)
+    kB = 1.380649e-16
+    i, j = 7, 3
+    dv = math.sqrt(8 * kB * T * (g.m_c[i] + g.m_c[j]) / (math.pi * g.m_c[i] * g.m_c[j]))
+    assert K[i, j] == pytest.approx(math.pi * (g.a_c[i] + g.a_c[j]) ** 2 * dv, rel=1e-12)
+    dv_eq = math.sqrt(16 * kB * T / (math.pi * g.m_c[5]))
+    assert K[5, 5] == pytest.approx(math.pi * 4 * g.a_c[5] ** 2 * dv_eq, rel=1e-12)
+
+
+def test_kernel_laminar_dominates_when_large():
+    """Eq. 57: the three contributions add in quadrature; with a huge imposed drift the relative
+    velocity is the drift difference and K = sigma |dv_lam|."""
+    g, T, rho_g, Omega, alpha, vR, vZ, p = _cell(vscale=1e7)
+    K, pf, *_ = orc.cell_kernel(g, T, rho_g, Omega, alpha, vR, vZ, p)
+    i, j = 11, 2
+    dv = math.hypot(vR[i] - vR[j], vZ[i] - vZ[j])
+    assert K[i, j] == pytest.approx(math.pi * (g.a_c[i] + g.a_c[j]) ** 2 * dv, rel=1e-8)
+    assert pf[i, j] == pytest.approx(1.0, abs=1e-8)
+    # azimuthal component enters the same way when supplied
+    vphi = np.zeros(g.N); vphi[i] = 3e7
+    K2, *_ = orc.cell_kernel(g, T, rho_g, Omega, alpha, vR, vZ, p, vphi=vphi)
+    dv2 = math.sqrt(dv * dv + 9e14)
+    assert K2[i, j] == pytest.approx(math.pi * (g.a_c[i] + g.a_c[j]) ** 2 * dv2, rel=1e-8)
+
+
+def test_kernel_quadrature_decomposition():
+    """dv^2 recovered from K must equal BM^2 + turb^2 + lam^2 assembled independently here
+    (Eqs. 56-60, Eq. 14 for St), including the Reynolds number chain of DESIGN.md R6."""
+    g, T, rho_g, Omega, alpha, vR, vZ, p = _cell(N=30, T=60.0, rho_g=3e-13, alpha=3e-3)
+    K, pf, St, Ss = orc.cell_kernel(g, T, rho_g, Omega, alpha, vR, vZ, p)
+    kB, mH = 1.380649e-16, 1.6735575e-24
+    cs = math.sqrt(kB * T / (p.mu * mH))
+    vth = math.sqrt(8 / math.pi) * cs
+    assert np.allclose(St, g.rho_m * g.a_c * Omega / (rho_g * vth), rtol=1e-14)      # Eq. 14
+    Re = (alpha * cs * cs / Omega) / (0.5 * vth * p.mu * mH / (rho_g * p.sigma_mol))
+    St_eta = Re ** -0.5
+    for (i, j) in ((29, 0), (15, 14), (8, 8), (22, 5)):
+        bm2 = 8 * kB * T * (g.m_c[i] + g.m_c[j]) / (math.pi * g.m_c[i] * g.m_c[j])
+        tb2 = alpha * cs * cs * orc.vrel2_turb(St[i], St[j], orc.ststar(St[i], St_eta), St_eta)
+        lm2 = (vR[i] - vR[j]) ** 2 + (vZ[i] - vZ[j]) ** 2
+        dv = math.sqrt(bm2 + tb2 + lm2)
+        assert K[i, j] == pytest.approx(math.pi * (g.a_c[i] + g.a_c[j]) ** 2 * dv, rel=1e-13)
+        assert pf[i, j] == pytest.approx(orc.pfrag(p.v_frag, dv), rel=1e-12, abs=1e-300)
+    assert np.all((Ss >= min(St_eta, 1.0) * (1 - 1e-13)) & (Ss <= 1.0))
+    assert Ss.min() == pytest.approx(St_eta, rel=1e-13)     # small grains sit on the Re^-1/2 floor
+
+
+# ---------------------------------------------------------------------------------- Eqs. 63-65
+def test_split_identities_and_brute_force():
+    g = orc.mass_grid(16, 1e-4, 1e-1, 1.0)
+    rng = np.random.default_rng(3)
+    for _ in range(500):
+        m = g.m_c[0] * (g.m_c[-1] / g.m_c[0]) ** rng.uniform(0, 1)
+        l, eps = orc.split(g, m)
+        # brute force l(m): largest index with m_l <= m
+        l_bf = max(k for k in range(g.N) if g.m_c[k] <= m)
+        assert l == l_bf and 0.0 <= eps <= 1.0
+        if l < g.N - 1:
+            # the two weights sum to one and interpolate the mass linearly (Eq. 65)
+            assert eps * g.m_c[l] + (1 - eps) * g.m_c[l + 1] == pytest.approx(m, rel=1e-13)
+    # exactly on a grid mass: everything into that bin (R7)
+    assert orc.split(g, g.m_c[5]) == (5, 1.0)
+    # off the grid (R8)
+    assert orc.split(g, g.m_c[-1] * 3) == (g.N - 1, 1.0)
+    assert orc.split(g, g.m_c[0] * 0.3) == (-1, 0.0)
+
+
+def test_lbin_is_smallest_l_with_upper_edge_above():
+    g = orc.mass_grid(16, 1e-4, 1e-1, 1.0)
+    rng = np.random.default_rng(4)
+    for _ in range(300):
+        m = g.m_e[0] * (g.m_e[-1] / g.m_e[0]) ** rng.uniform(0, 0.999)
+        l = orc.lbin(g, m)
+        assert l == min(k for k in range(g.N) if g.m_e[k + 1] > m)
+    for k in range(g.N):
+        assert orc.lbin(g, g.m_c[k]) == k         # a grid mass belongs to its own bin
