@@ -1,0 +1,183 @@
+/*
+ * cudisc_coag.h -- C ABI of libcudisc_coag.so: the per-cell Smoluchowski coagulation /
+ * fragmentation update of cuDisc (arXiv 2402.18471, section 5) as
+ * hand-written FP64 CUDA kernels for sm_100a (NVIDIA B200).
+ *
+ * Conventions
+ *   - All floating point is FP64, all quantities CGS.
+ *   - C = n_r * n_z cells, N = n_bins mass bins, P = N (N + 1) / 2 unordered pairs (i >= j).
+ *   - Every [C x N] array is row-major, bin fastest; cell index c = i_R * n_z + j_Z.
+ *   - "DEVICE" pointers are caller-owned CUDA device buffers (e.g. a torch tensor's data_ptr());
+ *     the library never frees or reallocates them.  "HOST" pointers are plain host memory.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  The three
+ *     hot calls only enqueue work on `stream` and return; they do not allocate and do not
+ *     synchronise with the host.
+ *   - Every function returns a cudisc_status.  No C++ exception crosses the ABI.
+ *     cudisc_last_error() returns a thread-local, NUL-terminated description of the last
+ *     non-zero status returned on the calling thread.
+ *   - Non-finite inputs are not checked on the hot path; NaN propagates into the outputs
+ *     (err_out in particular).
+ *   - There is no CPU fallback: without a CUDA device every call that needs one returns
+ *     CUDISC_ERR_CUDA.
+ *
+ * Readings of the paper where it is silent or garbled are listed in DESIGN.md ("Readings",
+ * R1..R16) and referenced below.
+ */
+#ifndef CUDISC_COAG_H
+#define CUDISC_COAG_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CUDISC_OK = 0,
+    CUDISC_ERR_INVALID = 1,     /* NULL pointer, n_bins < 2, a_min >= a_max, non-monotone masses ... */
+    CUDISC_ERR_HANDLE = 2,      /* bad handle, or grid was created for different bins             */
+    CUDISC_ERR_CUDA = 3,        /* CUDA runtime error (launch failure, no device, sticky error)   */
+    CUDISC_ERR_UNSUPPORTED = 4  /* size outside what the kernels support (n_bins > 256)           */
+} cudisc_status;
+
+typedef struct cudisc_bins_s *cudisc_bins;   /* mass grid + grid-only tables; owned by the library */
+typedef struct cudisc_grid_s *cudisc_grid;   /* cell grid: bound gas state, FSAL buffer, scratch   */
+typedef void *cudisc_stream;                 /* cudaStream_t */
+
+/* Physical / numerical parameters, passed by value. */
+typedef struct {
+    double mu;           /* mean molecular weight of the gas (default 2.4)          */
+    double v_frag;       /* fragmentation threshold velocity, cm/s (Eq. 62)         */
+    double alpha;        /* turbulent alpha used when gas_state.alpha == NULL      */
+    double eta;          /* fragment power-law slope (Eq. 66; default 11/6)         */
+    double chi_im;       /* fragment mass in units of the impactor mass (default 1) */
+    double sigma_mol;    /* H2 collision cross-section for nu_mol, cm^2 (reading R6; 2e-15)       */
+    double rtol;         /* BS3(2) relative tolerance (default 1e-2)                */
+    double atol_factor;  /* absolute tolerance = atol_factor * sum_k rho_k (1e-10)  */
+} cudisc_params;
+
+/* Frozen per-cell inputs from the other solvers.  DEVICE pointers. */
+typedef struct {
+    const double *T;        /* [C]  gas temperature, K                                            */
+    const double *rho_gas;  /* [C]  gas density, g/cm^3                                           */
+    const double *Omega;    /* [C]  Keplerian angular frequency, 1/s                              */
+    const double *alpha;    /* [C]  or NULL -> params.alpha in every cell                         */
+    const double *v_R;      /* [C x N] dust radial velocity per size, cm/s                        */
+    const double *v_Z;      /* [C x N] dust vertical velocity per size, cm/s                      */
+    const double *v_phi;    /* [C x N] or NULL (term left out of Delta v_lam)                     */
+} cudisc_gas_state;
+
+/* ---------------------------------------------------------------------------------------------
+ * Handles
+ * ------------------------------------------------------------------------------------------- */
+
+/* Mass grid of PAPER.md:442, 467, 503: n_bins bins <-> n_bins + 1 log-spaced edges in grain
+ * radius over [a_min, a_max] (cm); m^e_k = (4 pi / 3) rho_m (a^e_k)^3; centres are geometric
+ * means of the edges.  Also builds every grid-only table of the rate evaluation (two-bin split
+ * of Eqs. 63-65, remnant / fragment masses of Eq. 68, l-bins and N_k of Eq. 67) from p.eta and
+ * p.chi_im, on the host; they are uploaded to the current CUDA device on first use.
+ * p is stored: cudisc_coag_step uses it.  Works without a CUDA device (tables stay on the host).
+ * Errors: INVALID (n_bins < 2, a_min <= 0, a_min >= a_max, rho_m <= 0, eta >= 2, chi_im <= 0,
+ * out == NULL), UNSUPPORTED (n_bins > 256). */
+int cudisc_bins_create(int n_bins, double a_min, double a_max, double rho_m,
+                       cudisc_params p, cudisc_bins *out);
+
+/* Same for an arbitrary monotone mass grid: m_centres [n_bins], m_edges [n_bins + 1] (HOST,
+ * copied), strictly increasing with m_edges[k] < m_centres[k] < m_edges[k+1].  Grain radii are
+ * a_k = (3 m_k / (4 pi rho_m))^(1/3). */
+int cudisc_bins_create_general(int n_bins, const double *m_centres, const double *m_edges,
+                               double rho_m, cudisc_params p, cudisc_bins *out);
+
+int cudisc_bins_destroy(cudisc_bins b);
+
+/* Introspection of the host tables (HOST output pointers, any may be NULL):
+ *   m_centres [N], m_edges [N+1], a_centres [N]; n_bulk [N] = number of leading impactor bins j
+ *   of target row i whose collision outcomes are handled by the structured ("bulk") row sums;
+ *   *n_band = number of entries of the band gather lists (all remaining pair outcomes). */
+int cudisc_bins_query(cudisc_bins b, int *n_bins, double *m_centres, double *m_edges,
+                      double *a_centres, int *n_bulk, int *n_band);
+
+/* The full outcome table in gather form, for checking the host logic without a GPU.
+ * For every output bin k the rate is
+ *   drho_k = sum_e  coef[e] * n_{i[e]} * n_{j[e]} * Kplane[e]_{i[e] j[e]}     (entries with target k)
+ *          + A_k * sum_{l >= k} S_l / B_l,      S_l = same form over the S-entries with target l,
+ * where the lists returned here are the EXPANDED ones (bulk row/column sums written out pair by
+ * pair), so that a test can evaluate them with plain loops.  Call with all pointers NULL to get
+ * the counts.  target < N: density bin; target >= N: S bin (target - N).  plane 0 = K p_coag,
+ * 1 = K p_frag; the diagonal factor 1/2 is already folded into coef.
+ * frag_A [N], frag_invB [N]: A_k and 1 / B_l of PAPER.md:465-469. */
+int cudisc_bins_expand_outcomes(cudisc_bins b, long long *n_entries, int *target, int *i, int *j,
+                                int *plane, double *coef, double *frag_A, double *frag_invB);
+
+/* Cell grid of n_r x n_z cells using mass grid b.  Allocates on the current CUDA device: the
+ * FSAL buffer [C x N], and the kernel scratch.  The handle remembers b. */
+int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out);
+
+/* Bind the frozen gas state used by cudisc_coag_step.  The struct is copied, the arrays are NOT:
+ * they must stay valid and unchanged while steps are enqueued.  Invalidates the FSAL buffer. */
+int cudisc_grid_bind_gas(cudisc_grid g, const cudisc_gas_state *gs);
+
+/* Invalidate the saved last-stage derivative k4 (call after changing rho_dust outside the
+ * library, or the gas arrays in place): the next step recomputes k1 = f(rho). */
+int cudisc_grid_reset_fsal(cudisc_grid g);
+
+int cudisc_grid_destroy(cudisc_grid g);
+
+/* ---------------------------------------------------------------------------------------------
+ * Hot path
+ * ------------------------------------------------------------------------------------------- */
+
+/* Collision kernel of every cell, PAPER.md:410-440 (Eqs. 55-62): K_ij = sigma_ij dv_ij with
+ * sigma_ij = pi (a_i + a_j)^2 (R3), dv_ij^2 = Brownian (Eq. 58) + turbulent (Eqs. 59-60, Ormel &
+ * Cuzzi 2007 closed forms, R4) + laminar (v_R, v_Z [, v_phi] differences), and the
+ * fragmentation probability p_frag of Eq. 62.
+ * K_out: DEVICE [C][2][P], packed lower-triangular (i >= j at index i (i + 1) / 2 + j):
+ *        plane 0 = K_ij (1 - p_frag,ij), plane 1 = K_ij p_frag,ij; the diagonal is NOT halved.
+ * Uses p.mu, p.v_frag, p.alpha (if gs->alpha == NULL) and p.sigma_mol; gs must be non-NULL. */
+int cudisc_coag_kernel(cudisc_grid g, cudisc_bins b, const cudisc_gas_state *gs,
+                       cudisc_params p, double *K_out, cudisc_stream stream);
+
+/* Rate evaluation from a supplied kernel, PAPER.md:396-404, 432-476 (Eqs. 53, 54, 61-68) in the
+ * cancellation-free pair-flux form (R9): drho_dt_k for every cell.
+ * K: DEVICE [C][2][P] as written by cudisc_coag_kernel -- ANY symmetric kernel is accepted
+ *    (closed-form tests pass plane 0 = K, plane 1 = 0).
+ * rho_dust: DEVICE [C x N] in; drho_dt: DEVICE [C x N] out.  May not alias. */
+int cudisc_coag_rates(cudisc_grid g, cudisc_bins b, const double *K,
+                      const double *rho_dust, double *drho_dt, cudisc_stream stream);
+
+/* Extension: the same rate evaluation with K built on the fly from the gas state bound to g
+ * (never written to HBM). */
+int cudisc_coag_rates_otf(cudisc_grid g, cudisc_bins b, const double *rho_dust, double *drho_dt,
+                          cudisc_stream stream);
+
+/* One Bogacki-Shampine 3(2) step of size dt (s) of every cell, with the kernel
+ * built on the fly, once per cell per step, from the gas state bound to g and frozen over the
+ * stages; parameters are those given to cudisc_bins_create.
+ * rho_dust: DEVICE [C x N] in/out.  err_out: DEVICE [C], the scaled error norm of each cell
+ *   E_c = max_k |e_k| / (atol_factor * sum_k rho_k + rtol * max(|rho_k|, |rho_k^new|))   (R10);
+ * the step is accepted by the caller iff max_c E_c <= 1 (this call always advances rho_dust).
+ * The first call after create / bind_gas / reset_fsal evaluates k1 = f(rho) (4 rate evaluations);
+ * later calls reuse the saved k4 (FSAL, 3 evaluations). */
+int cudisc_coag_step(cudisc_grid g, cudisc_bins b, double *rho_dust, double dt,
+                     double *err_out, cudisc_stream stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Roofline denominators measured in the same process (north_star: "peaks measured by a
+ * microbenchmark in the same run").  Both synchronise the device.
+ * ------------------------------------------------------------------------------------------- */
+
+/* Dependent-chain-free DFMA loop on every SM: *dfma_per_s = FP64 fused multiply-adds per second
+ * (thread-level operations).  n_iter <= 0 picks a default that runs for ~50 ms. */
+int cudisc_microbench_dfma(int n_iter, double *dfma_per_s, double *elapsed_ms);
+
+/* STREAM-style device copy of n_bytes (read + write counted): *bytes_per_s. */
+int cudisc_microbench_copy(long long n_bytes, double *bytes_per_s, double *elapsed_ms);
+
+/* Number of kernels this library has launched in this process (bench.py's gpu_launches). */
+long long cudisc_launch_count(void);
+
+const char *cudisc_last_error(void);
+const char *cudisc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CUDISC_COAG_H */

@@ -1,0 +1,23 @@
+// coag_launch.h -- internal interface between the C-ABI layer (coag_api.cu) and the kernels.
+#pragma once
+#include "coag_device.cuh"
+
+namespace cudisc {
+
+constexpr int kThreads = 512;   // threads per CTA of the cell kernels
+
+struct LaunchCfg {
+    int grid;            // persistent CTAs
+    int smem_bytes;      // dynamic shared memory of this launch
+    int smem_optin;      // device limit (cudaDevAttrMaxSharedMemoryPerBlockOptin)
+};
+
+// mode: 0 kernel, 1 rates (supplied K), 2 rates on the fly, 3 BS3(2) step
+cudaError_t launch_cells(int mode, const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
+                         const StepArgs &sa, cudaStream_t st);
+// resident CTAs per SM of the cell kernels with `smem_bytes` of dynamic shared memory (0 on error)
+int cells_occupancy(int smem_bytes, int smem_optin);
+cudaError_t launch_dfma_peak(int grid, int n_iter, double *out, cudaStream_t st);
+cudaError_t launch_copy_peak(int grid, const void *src, void *dst, size_t n16, cudaStream_t st);
+
+}  // namespace cudisc

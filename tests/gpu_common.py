@@ -1,0 +1,111 @@
+"""Shared plumbing of the -m gpu parity tests: moves seeded inputs to the device, calls the CUDA
+path through the C-ABI binding, calls the oracle on the same inputs.  No method arithmetic."""
+import json
+import os
+
+import numpy as np
+
+import oracle as orc
+import paper_2402_18471_b200 as cd
+from paper_2402_18471_b200 import synth_disc
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+# Tolerances (BASELINE.json north_star)
+TOL_K = 1e-12          # |dKc|, |dKf| <= TOL_K * K_ij
+TOL_RATE = 1e-11       # |d drho_k| <= TOL_RATE * (gain_k + loss_k)
+TOL_RHO_1 = 1e-11      # one step, relative, bins with rho_k > 1e-30 sum(rho)
+TOL_RHO_100 = 1e-9     # after 100 steps
+TOL_MASS = 1e-13       # relative drift of sum_k rho_k per step
+
+
+def dt_of(index: int) -> float:
+    with open(os.path.join(ROOT, "tests", "golden", "dt_manifest.json")) as f:
+        return float(json.load(f)[str(index)]["dt_s"])
+
+
+def params_pair(cfg):
+    po = orc.Params(mu=cfg.mu, v_frag=cfg.v_frag, eta=cfg.eta, chi_im=cfg.chi_im, sigma_mol=cfg.sigma_mol)
+    pc = cd.Params(mu=cfg.mu, v_frag=cfg.v_frag, alpha=cfg.alpha, eta=cfg.eta, chi_im=cfg.chi_im,
+                   sigma_mol=cfg.sigma_mol)
+    return po, pc
+
+
+class GpuDisc:
+    """Device copy of a DiscInputs plus the library handles."""
+
+    def __init__(self, d, pc, n_r=None, n_z=None, use_alpha_array=True, v_phi=None):
+        import torch
+        self.torch = torch
+        self.d = d
+        self.pc = pc
+        dev = torch.device("cuda:0")
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        self.gas = dict(T=t(d.T), rho_gas=t(d.rho_gas), Omega=t(d.Omega), v_R=t(d.v_R), v_Z=t(d.v_Z),
+                        alpha=t(d.alpha) if use_alpha_array else None,
+                        v_phi=t(v_phi) if v_phi is not None else None)
+        self.rho = t(d.rho_dust)
+        self.bins = cd.Bins(d.n_bins, d.a_min, d.a_max, d.rho_m, pc)
+        C = d.n_cells
+        if n_r is None:
+            n_r, n_z = C, 1
+        self.grid = cd.Grid(n_r, n_z, self.bins)
+        self.grid.bind_gas(**self.gas)
+        self.C, self.N, self.P = C, d.n_bins, self.bins.n_pairs
+
+    def kernel(self):
+        K = self.torch.empty((self.C, 2, self.P), dtype=self.torch.float64, device="cuda:0")
+        cd.cudisc_coag_kernel(self.grid, self.bins, self.gas, self.pc, K)
+        self.torch.cuda.synchronize()
+        return K
+
+    def rates(self, K, rho=None):
+        rho = self.rho if rho is None else rho
+        out = self.torch.empty_like(rho)
+        cd.cudisc_coag_rates(self.grid, self.bins, K, rho, out)
+        self.torch.cuda.synchronize()
+        return out
+
+    def rates_otf(self, rho=None):
+        rho = self.rho if rho is None else rho
+        out = self.torch.empty_like(rho)
+        cd.cudisc_coag_rates_otf(self.grid, self.bins, rho, out)
+        self.torch.cuda.synchronize()
+        return out
+
+    def step(self, rho, dt):
+        err = self.torch.empty(self.C, dtype=self.torch.float64, device="cuda:0")
+        cd.cudisc_coag_step(self.grid, self.bins, rho, dt, err)
+        self.torch.cuda.synchronize()
+        return err
+
+
+def oracle_args(d):
+    return (d.n_bins, d.a_min, d.a_max, d.rho_m, d.T, d.rho_gas, d.Omega, d.alpha, d.v_R, d.v_Z)
+
+
+def assert_rho_close(rho_gpu, rho_ref, tol, what=""):
+    """relative per-bin parity on bins with |rho_k| > 1e-30 * cell total (north_star)."""
+    tot = rho_ref.sum(axis=1, keepdims=True)
+    mask = np.abs(rho_ref) > 1e-30 * tot
+    rel = np.abs(rho_gpu - rho_ref) / np.where(mask, np.abs(rho_ref), 1.0)
+    rel = np.where(mask, rel, 0.0)
+    worst = np.unravel_index(np.argmax(rel), rel.shape)
+    assert rel.max() <= tol, f"{what}: max rel diff {rel.max():.3e} at cell/bin {worst} (tol {tol})"
+    # bins below the mask: must still be tiny
+    small = ~mask
+    if small.any():
+        assert np.all(np.abs(rho_gpu[small]) <= 1e-29 * np.broadcast_to(tot, rho_ref.shape)[small] + 1e-300), what
+    return rel.max()
+
+
+def assert_rates_close(d_gpu, d_ref, gain, loss, tol=TOL_RATE, what=""):
+    scale = gain + loss
+    diff = np.abs(d_gpu - d_ref)
+    bad = diff > tol * scale
+    if bad.any():
+        w = np.unravel_index(np.argmax(diff / np.where(scale > 0, scale, 1.0)), diff.shape)
+        raise AssertionError(f"{what}: {bad.sum()} bins off; worst at {w}: gpu {d_gpu[w]:.17e} ref {d_ref[w]:.17e} "
+                             f"gain+loss {scale[w]:.3e}")
+    nz = scale > 0
+    return float((diff[nz] / scale[nz]).max()) if nz.any() else 0.0

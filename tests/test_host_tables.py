@@ -1,0 +1,104 @@
+"""Host logic of the CUDA library (no GPU): the C-ABI library loads, exports every symbol of
+include/cudisc_coag.h, validates arguments, and its grid-only outcome tables -- evaluated here with
+plain NumPy gathers -- reproduce the oracle's rate evaluation for random kernels and densities."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle as orc
+import paper_2402_18471_b200 as cd
+from paper_2402_18471_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "cudisc_coag.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(cudisc_[a-z_0-9]+)\s*\(", hdr))
+    assert declared, "no declarations parsed"
+    L = cd.lib()
+    for name in sorted(declared):
+        assert hasattr(L, name), f"{name} declared in include/cudisc_coag.h but not exported"
+    assert declared == set(binding.EXPORTS)
+    assert "sm_100a" in cd.cudisc_version()
+
+
+def test_argument_validation_without_gpu():
+    p = cd.Params()
+    for bad in [dict(n_bins=1, a_min=1e-5, a_max=1.0, rho_m=1.67),
+                dict(n_bins=10, a_min=1.0, a_max=1e-5, rho_m=1.67),
+                dict(n_bins=10, a_min=1e-5, a_max=1.0, rho_m=-1.0)]:
+        with pytest.raises(cd.CudiscError) as ei:
+            cd.Bins(params=p, **bad)
+        assert ei.value.code == 1
+    with pytest.raises(cd.CudiscError) as ei:
+        cd.Bins(300, 1e-5, 1.0, 1.67, p)
+    assert ei.value.code == 4
+    with pytest.raises(cd.CudiscError) as ei:
+        cd.Bins(10, 1e-5, 1.0, 1.67, cd.Params(eta=2.5))
+    assert ei.value.code == 1
+    # bad handle
+    assert cd.lib().cudisc_bins_destroy(None) == 2
+    assert b"handle" in cd.lib().cudisc_last_error()
+
+
+def test_mass_grid_matches_paper_ratio_and_oracle_grid():
+    b = cd.Bins(100, 1e-5, 0.5, 1.67, cd.Params())
+    q = b.query()
+    ratio = q["m_centres"][1:] / q["m_centres"][:-1]
+    assert f"{ratio.mean():.2f}" == "1.38"
+    g = orc.mass_grid(100, 1e-5, 0.5, 1.67)
+    np.testing.assert_allclose(q["m_centres"], g.m_c, rtol=1e-14)
+    np.testing.assert_allclose(q["m_edges"], g.m_e, rtol=1e-14)
+    np.testing.assert_allclose(q["a_centres"], g.a_c, rtol=1e-14)
+
+
+def _eval_tables(ex, N, Kc, Kf, rho, m_c):
+    n = rho / m_c
+    planes = np.stack([Kc, Kf])
+    contrib = ex["coef"] * n[ex["i"]] * n[ex["j"]] * planes[ex["plane"], ex["i"], ex["j"]]
+    acc = np.zeros(2 * N)
+    np.add.at(acc, ex["target"], contrib)
+    d = acc[:N].copy()
+    S = acc[N:]
+    suffix = np.cumsum((S * ex["frag_invB"])[::-1])[::-1]
+    d += ex["frag_A"] * suffix
+    return d, S
+
+
+@pytest.mark.parametrize("N,a_max,chi", [(40, 1.0, 1.0), (100, 10.0, 1.0), (150, 10.0, 1.0),
+                                         (24, 1e-1, 0.4), (30, 1e-2, 2.5), (12, 1e-4, 1.0), (2, 2e-5, 1.0)])
+def test_outcome_tables_reproduce_oracle_rates(N, a_max, chi):
+    rng = np.random.default_rng(N * 7 + int(chi * 10))
+    p = cd.Params(chi_im=chi)
+    b = cd.Bins(N, 1e-5, a_max, 1.67, p)
+    ex = b.expand_outcomes()
+    g = orc.mass_grid(N, 1e-5, a_max, 1.67)
+    K = rng.uniform(0.5, 2.0, size=(N, N)); K = 0.5 * (K + K.T)
+    pf = rng.uniform(0.0, 1.0, size=(N, N)); pf = 0.5 * (pf + pf.T)
+    rho = 10.0 ** rng.uniform(-3, 0, size=N)
+    d_ref, gain, loss, S_ref = orc.rates_flux(g, K, pf, rho, chi=chi)
+    d, S = _eval_tables(ex, N, K * (1 - pf), K * pf, rho, g.m_c)
+    np.testing.assert_allclose(S, S_ref, rtol=1e-12, atol=1e-300)
+    assert np.all(np.abs(d - d_ref) <= 1e-12 * (gain + loss))
+    # bulk prefixes exist on fine grids and are absent above the diagonal
+    nb = b.query()["n_bulk"]
+    assert np.all(nb <= np.arange(N) + 1)
+    if N >= 100:
+        assert nb[-1] > N - 12
+
+
+def test_general_grid_tables_match_log_grid_tables():
+    N = 50
+    p = cd.Params()
+    b1 = cd.Bins(N, 1e-5, 1.0, 1.67, p)
+    q = b1.query()
+    b2 = cd.Bins(N, 0, 0, 1.67, p, m_centres=q["m_centres"], m_edges=q["m_edges"])
+    e1, e2 = b1.expand_outcomes(), b2.expand_outcomes()
+    for k in e1:
+        np.testing.assert_array_equal(e1[k], e2[k])
+    np.testing.assert_allclose(b2.query()["a_centres"], q["a_centres"], rtol=1e-14)
