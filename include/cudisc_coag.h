@@ -159,6 +159,18 @@ int cudisc_coag_rates_otf(cudisc_grid g, cudisc_bins b, const double *rho_dust, 
 int cudisc_coag_step(cudisc_grid g, cudisc_bins b, double *rho_dust, double dt,
                      double *err_out, cudisc_stream stream);
 
+/* End-to-end form of cudisc_coag_step for callers whose dust array lives in HOST memory (the
+ * other solvers of the paper's global loop, when they run elsewhere):
+ * rho_host: HOST [C x N] in/out, err_host: HOST [C] out (page-locked memory makes the copies
+ * asynchronous and full-speed; pageable memory works).  Enqueues on `stream`: host->device copy
+ * of rho_host into a staging buffer owned by g (allocated on the first call, the only allocation
+ * this call ever makes), the same kernel as cudisc_coag_step, device->host copies of the new
+ * densities and of the error norms; then WAITS for the stream, so the host buffers are valid on
+ * return.  The FSAL derivative is kept on the device exactly as for cudisc_coag_step: call
+ * cudisc_grid_reset_fsal if rho_host was modified between steps. */
+int cudisc_coag_step_host(cudisc_grid g, cudisc_bins b, double *rho_host, double dt,
+                          double *err_host, cudisc_stream stream);
+
 /* ---------------------------------------------------------------------------------------------
  * Roofline denominators measured in the same process (north_star: "peaks measured by a
  * microbenchmark in the same run").  Both synchronise the device.

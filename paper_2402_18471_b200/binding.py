@@ -40,7 +40,7 @@ EXPORTS = [
     "cudisc_bins_create", "cudisc_bins_create_general", "cudisc_bins_destroy", "cudisc_bins_query",
     "cudisc_bins_expand_outcomes", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
     "cudisc_grid_destroy", "cudisc_coag_kernel", "cudisc_coag_rates", "cudisc_coag_rates_otf",
-    "cudisc_coag_step", "cudisc_microbench_dfma",
+    "cudisc_coag_step", "cudisc_coag_step_host", "cudisc_microbench_dfma",
     "cudisc_microbench_copy", "cudisc_launch_count", "cudisc_last_error", "cudisc_version",
 ]
 
@@ -69,6 +69,7 @@ def lib() -> C.CDLL:
         L.cudisc_coag_rates.argtypes = [vp, vp, vp, vp, vp, vp]
         L.cudisc_coag_rates_otf.argtypes = [vp, vp, vp, vp, vp]
         L.cudisc_coag_step.argtypes = [vp, vp, vp, C.c_double, vp, vp]
+        L.cudisc_coag_step_host.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.cudisc_microbench_dfma.argtypes = [C.c_int, dp, dp]
         L.cudisc_microbench_copy.argtypes = [C.c_longlong, dp, dp]
         L.cudisc_launch_count.restype = C.c_longlong
@@ -248,6 +249,26 @@ def cudisc_coag_step(grid: Grid, bins: Bins, rho_dust, dt: float, err_out, strea
     Cn, N = grid.n_cells, bins.n_bins
     _check(lib().cudisc_coag_step(grid.handle, bins.handle, _dev_ptr(rho_dust, "rho_dust", Cn * N),
                                   float(dt), _dev_ptr(err_out, "err_out", Cn), _stream(stream)))
+
+
+def _host_ptr(t, name: str, numel: int) -> int:
+    import torch
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.float64 or not t.flags.c_contiguous or t.size != numel:
+            raise TypeError(f"{name}: expected a C-contiguous float64 array of {numel} elements")
+        return t.ctypes.data
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() \
+            or t.numel() != numel:
+        raise TypeError(f"{name}: expected a contiguous float64 HOST tensor of {numel} elements")
+    return t.data_ptr()
+
+
+def cudisc_coag_step_host(grid: Grid, bins: Bins, rho_host, dt: float, err_host, stream=None) -> None:
+    """cudisc_coag_step with HOST buffers (pinned torch tensors or numpy arrays): H2D copy, step,
+    D2H copies, stream wait -- all inside the library call."""
+    Cn, N = grid.n_cells, bins.n_bins
+    _check(lib().cudisc_coag_step_host(grid.handle, bins.handle, _host_ptr(rho_host, "rho_host", Cn * N),
+                                       float(dt), _host_ptr(err_host, "err_host", Cn), _stream(stream)))
 
 
 def cudisc_microbench_dfma(n_iter: int = 0):

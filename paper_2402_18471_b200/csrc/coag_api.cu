@@ -61,6 +61,8 @@ struct cudisc_grid_s {
     bool fsal_valid;
     double *k_fsal;     // [C x N]
     double *kslab;      // per-CTA overflow of the K store
+    double *stage_rho;  // [C x N] staging of cudisc_coag_step_host (lazy)
+    double *stage_err;  // [C]
     int num_sms, smem_optin, grid_ctas, Psm, smem_bytes;
 };
 
@@ -328,6 +330,7 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
     g->bins = b;
     g->gas_bound = false; g->fsal_valid = false;
     g->k_fsal = nullptr; g->kslab = nullptr;
+    g->stage_rho = nullptr; g->stage_err = nullptr;
     g->num_sms = sms; g->smem_optin = optin;
 
     const DevTables &d = b->dt;
@@ -379,6 +382,8 @@ int cudisc_grid_destroy(cudisc_grid g)
     if (!g || g->magic != kGridMagic) return fail(CUDISC_ERR_HANDLE, "bad grid handle");
     if (g->k_fsal) cudaFree(g->k_fsal);
     if (g->kslab) cudaFree(g->kslab);
+    if (g->stage_rho) cudaFree(g->stage_rho);
+    if (g->stage_err) cudaFree(g->stage_err);
     g->magic = 0;
     delete g;
     return CUDISC_OK;
@@ -444,6 +449,35 @@ int cudisc_coag_step(cudisc_grid g, cudisc_bins b, double *rho_dust, double dt, 
     rc = run(g, 3, gas_args(g->gs, b->p), sa, stream);
     if (rc == CUDISC_OK) g->fsal_valid = true;
     return rc;
+}
+
+int cudisc_coag_step_host(cudisc_grid g, cudisc_bins b, double *rho_host, double dt,
+                          double *err_host, cudisc_stream stream)
+{
+    int rc = check_pair(g, b);
+    if (rc) return rc;
+    if (!rho_host || !err_host) return fail(CUDISC_ERR_INVALID, "NULL array argument");
+    const size_t row_bytes = (size_t)g->C * b->ht.N * sizeof(double);
+    const size_t err_bytes = (size_t)g->C * sizeof(double);
+    cudaError_t e = cudaSuccess;
+    if (!g->stage_rho) {
+        e = cudaMalloc((void **)&g->stage_rho, row_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g->stage_err, err_bytes);
+        if (e != cudaSuccess) {
+            if (g->stage_rho) { cudaFree(g->stage_rho); g->stage_rho = nullptr; }
+            return cuda_fail(e, "cudaMalloc(staging)");
+        }
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    e = cudaMemcpyAsync(g->stage_rho, rho_host, row_bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(H2D)");
+    rc = cudisc_coag_step(g, b, g->stage_rho, dt, g->stage_err, stream);
+    if (rc) return rc;
+    e = cudaMemcpyAsync(rho_host, g->stage_rho, row_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(err_host, g->stage_err, err_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(e, "step_host copies");
+    return CUDISC_OK;
 }
 
 int cudisc_microbench_dfma(int n_iter, double *dfma_per_s, double *elapsed_ms)
