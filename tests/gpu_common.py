@@ -87,6 +87,19 @@ def oracle_args(d):
     return (d.n_bins, d.a_min, d.a_max, d.rho_m, d.T, d.rho_gas, d.Omega, d.alpha, d.v_R, d.v_Z)
 
 
+def split_free_magnitudes(d, po, cfg):
+    """Gain and loss magnitudes of every bin with p_coag = p_frag = 1 (both planes = the oracle's
+    K_ij): the scale of the rate comparison when BOTH sides build the kernel themselves.  Eq. 55's
+    p_coag = 1 - p_frag carries an absolute rounding error u on either side, so K p_coag is only
+    good to u K_ij, not to u K_ij p_coag."""
+    Kref = orc.kernel_cells(*oracle_args(d), po)
+    Ktot = Kref[:, 0] + Kref[:, 1]
+    planes = np.ascontiguousarray(np.stack([Ktot, Ktot], axis=1))
+    _, gain, loss = orc.rates_cells_planes(d.n_bins, d.a_min, d.a_max, d.rho_m, planes, d.rho_dust,
+                                           eta=cfg.eta, chi=cfg.chi_im)
+    return gain, loss
+
+
 def assert_rho_close(rho_gpu, rho_ref, tol, what=""):
     """relative per-bin parity on bins with |rho_k| > 1e-30 * cell total (north_star)."""
     tot = rho_ref.sum(axis=1, keepdims=True)

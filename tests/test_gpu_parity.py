@@ -8,7 +8,7 @@ import paper_2402_18471_b200 as cd
 from paper_2402_18471_b200 import synth_disc
 
 from gpu_common import (TOL_K, TOL_MASS, TOL_RHO_1, TOL_RHO_100, GpuDisc, assert_rates_close,
-                        assert_rho_close, dt_of, oracle_args, params_pair)
+                        assert_rho_close, dt_of, oracle_args, params_pair, split_free_magnitudes)
 
 pytestmark = pytest.mark.gpu
 
@@ -70,7 +70,8 @@ def test_rates_on_the_fly_match_oracle(index, n_cells):
     cfg, d = _disc(index, n_cells)
     po, pc = params_pair(cfg)
     g = GpuDisc(d, pc)
-    dref, gain, loss = orc.rates_cells(*oracle_args(d), po, d.rho_dust)
+    dref, _, _ = orc.rates_cells(*oracle_args(d), po, d.rho_dust)
+    gain, loss = split_free_magnitudes(d, po, cfg)
     out = g.rates_otf().cpu().numpy()
     assert_rates_close(out, dref, gain, loss, what=f"cfg{index} rates_otf")
 
