@@ -3,6 +3,7 @@
 // kernels: coag_kernels.cu / coag_device.cuh).
 #include "../../include/cudisc_coag.h"
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
@@ -63,6 +64,7 @@ struct cudisc_grid_s {
     double *kslab;      // per-CTA overflow of the K store
     double *stage_rho;  // [C x N] staging of cudisc_coag_step_host (lazy)
     double *stage_err;  // [C]
+    long long *prof;    // CUDISC_PROF builds only
     int num_sms, smem_optin, grid_ctas, Psm, smem_bytes;
 };
 
@@ -122,24 +124,73 @@ int upload_tables(cudisc_bins b)
     d.N = N; d.Np = (N + 1) & ~1; d.P = N * (N + 1) / 2;
     d.rho_m = t.rho_m; d.sS = t.sS;
 
-    // row-pass items: (block of 32 rows, chunk of 32 impactors), heaviest first
-    std::vector<uint32_t> itemsA, itemsB;
-    int nchA = 1;
     const int nblk = (N + 31) / 32;
-    for (int blk = 0; blk < nblk; ++blk) {
-        int mx = 0;
-        for (int i = blk * 32; i < std::min(N, blk * 32 + 32); ++i) mx = std::max(mx, t.n_bulk[i]);
-        const int nch = (mx + 31) / 32;
-        nchA = std::max(nchA, nch);
-        for (int c = 0; c < nch; ++c) itemsA.push_back((uint32_t)blk | ((uint32_t)c << 16));
+
+    // ---- build items (all about equal: small items for balance), packed (coag_device.cuh)
+    std::vector<uint32_t> buildItems;
+    constexpr int kRowsPerItem = 4, kPairsPerItem = 64;
+    for (int c = 0; c < nblk; ++c)
+        for (int ia = 32 * c + 31; ia < N; ia += kRowsPerItem)
+            buildItems.push_back(pack_build(IT_BUILD_ROWS, c, ia, std::min(N, ia + kRowsPerItem)));
+    for (int c = 0; c < nblk; ++c) {
+        const int rows = std::min(32 * c + 31, N) - 32 * c;          // rows 32 c .. 32 c + rows - 1
+        const int last = rows * (rows + 1) / 2;
+        for (int a = 0; a < last; a += kPairsPerItem)
+            buildItems.push_back(pack_build(IT_BUILD_LIST, c, a, std::min(last, a + kPairsPerItem)));
     }
-    // column-pass items: (block of 32 columns cb, chunk r of 32 rows starting at the diagonal block)
-    const int nchB = nblk;
+
+    // ---- eval items: band gathers first (global-memory latency), then row / column passes by cost
+    const int nchRow = std::max(1, (N + kRowChunk - 1) / kRowChunk);
+    const int nRng = std::max(1, (N + 63) / 64);
+    const int rngLen = (N + nRng - 1) / nRng;
+    struct Cost { uint32_t item; long cost; };
+    std::vector<Cost> work;
+    for (int blk = 0; blk < nblk; ++blk)
+        for (int cw = 0; cw < nchRow; ++cw) {
+            int jmax = 0;
+            for (int i = blk * 32; i < std::min(N, blk * 32 + 32); ++i)
+                jmax = std::max(jmax, std::min(kRowChunk * cw + kRowChunk, t.n_bulk[i]));
+            if (jmax <= kRowChunk * cw) continue;
+            work.push_back({pack_eval(IT_ROW, blk, cw, 0, jmax), 5L * (jmax - kRowChunk * cw)});
+        }
     for (int cb = 0; cb < nblk; ++cb)
-        for (int r = 0; cb * 32 + r * 32 < N; ++r) itemsB.push_back((uint32_t)cb | ((uint32_t)r << 16));
-    d.nItemsA = (int)itemsA.size(); d.nItemsB = (int)itemsB.size();
-    d.nchA = nchA; d.nchB = nchB;
-    d.partStride = std::max(std::max(4 * nchA, 2 * nchB), 12);
+        for (int r = 0; r < nRng; ++r) {
+            const int i0 = r * rngLen, i1 = std::min(N, (r + 1) * rngLen);
+            if (i1 <= 32 * cb) continue;
+            work.push_back({pack_eval(IT_COL, cb, r, i0, i1), 5L * (i1 - std::max(i0, 32 * cb))});
+        }
+    std::stable_sort(work.begin(), work.end(), [](const Cost &x, const Cost &y) { return x.cost > y.cost; });
+    d.nchRow = nchRow; d.nRng = nRng; d.rngLen = rngLen;
+
+    // per-bin constants
+    std::vector<double> binc((size_t)kBinC * d.Np, 0.0);
+    std::vector<int2> bini(d.Np, make_int2(0, 0));
+    for (int k = 0; k < N; ++k) {
+        binc[(size_t)BC_M * d.Np + k] = t.m[k];   binc[(size_t)BC_RM * d.Np + k] = t.rm[k];
+        binc[(size_t)BC_A1 * d.Np + k] = t.cA1[k]; binc[(size_t)BC_A2 * d.Np + k] = t.cA2[k];
+        binc[(size_t)BC_B1 * d.Np + k] = t.cB1[k];
+        binc[(size_t)BC_F1 * d.Np + k] = t.cF1[k]; binc[(size_t)BC_F2 * d.Np + k] = t.cF2[k];
+        binc[(size_t)BC_G1 * d.Np + k] = t.cG1[k];
+        binc[(size_t)BC_FA * d.Np + k] = t.fA[k];  binc[(size_t)BC_FIB * d.Np + k] = t.finvB[k];
+        bini[k] = make_int2(t.n_bulk[k] | (t.iS[k] << 16), t.jS_lo[k] | (t.jS_hi[k] << 16));
+    }
+
+    // per-offset tables of a log grid: sigma_ij = a_i^2 pi (1 + q^-d)^2, (St_i - St_j)/(St_i + St_j)
+    // = (1 - q^-d)/(1 + q^-d) with q^-d = a_0 / a_d (Epstein Stokes numbers are proportional to a)
+    std::vector<double> dtab(2 * (size_t)N, 0.0), exptab(64);
+    {
+        const double q = std::pow(t.a[N - 1] / t.a[0], 1.0 / (double)(N - 1));
+        bool lg = true;
+        for (int k = 0; k + 1 < N; ++k)
+            if (std::fabs(t.a[k + 1] / t.a[k] - q) > 1e-12 * q) lg = false;
+        d.logGrid = lg ? 1 : 0;
+        for (int dd = 0; dd < N; ++dd) {
+            const double r = t.a[0] / t.a[dd];
+            dtab[2 * dd] = 3.14159265358979323846 * (1.0 + r) * (1.0 + r);
+            dtab[2 * dd + 1] = (1.0 - r) / (1.0 + r);
+        }
+        for (int qq = 0; qq < 64; ++qq) exptab[qq] = std::exp2((double)qq / 64.0);
+    }
 
     // band ELL: entries of target t at [e][t], e < band_cnt[t]
     const int W = (2 * N + 31) & ~31;
@@ -156,16 +207,20 @@ int upload_tables(cudisc_bins b)
         bcoef[(size_t)e2 * W + be.target] = be.coef;
     }
     d.bandW = W; d.bandL = L;
+    std::vector<uint32_t> evalItems;
+    for (int tg = 0; tg * 32 < 2 * N; ++tg) {
+        int cmax = 0;
+        for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
+        evalItems.push_back(pack_eval(IT_BAND, tg, 0, 0, cmax));
+    }
+    for (const Cost &c : work) evalItems.push_back(c.item);
+    d.nBuildItems = (int)buildItems.size(); d.nEvalItems = (int)evalItems.size();
 
     Blob bl;
-    const size_t o_m = bl.add(t.m), o_rm = bl.add(t.rm), o_a = bl.add(t.a);
-    const size_t o_cA1 = bl.add(t.cA1), o_cA2 = bl.add(t.cA2), o_cB1 = bl.add(t.cB1), o_cB2 = bl.add(t.cB2);
-    const size_t o_cF1 = bl.add(t.cF1), o_cF2 = bl.add(t.cF2), o_cG1 = bl.add(t.cG1), o_cG2 = bl.add(t.cG2);
-    const size_t o_nb = bl.add(t.n_bulk), o_iS = bl.add(t.iS), o_lj = bl.add(t.lj);
-    const size_t o_jlo = bl.add(t.jS_lo), o_jhi = bl.add(t.jS_hi);
-    const size_t o_fA = bl.add(t.fA), o_fB = bl.add(t.finvB);
+    const size_t o_a = bl.add(t.a), o_binc = bl.add(binc), o_bini = bl.add(bini);
     const size_t o_cnt = bl.add(cnt), o_bidx = bl.add(bidx), o_bcoef = bl.add(bcoef);
-    const size_t o_iA = bl.add(itemsA), o_iB = bl.add(itemsB);
+    const size_t o_bI = bl.add(buildItems), o_eI = bl.add(evalItems);
+    const size_t o_dt = bl.add(dtab), o_ex = bl.add(exptab);
 
     void *blob = nullptr;
     e = cudaMalloc(&blob, bl.bytes.size());
@@ -173,17 +228,12 @@ int upload_tables(cudisc_bins b)
     e = cudaMemcpy(blob, bl.bytes.data(), bl.bytes.size(), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(blob); return cuda_fail(e, "cudaMemcpy(tables)"); }
     const unsigned char *base = (const unsigned char *)blob;
-    d.m = (const double *)(base + o_m); d.rm = (const double *)(base + o_rm); d.a = (const double *)(base + o_a);
-    d.cA1 = (const double *)(base + o_cA1); d.cA2 = (const double *)(base + o_cA2);
-    d.cB1 = (const double *)(base + o_cB1); d.cB2 = (const double *)(base + o_cB2);
-    d.cF1 = (const double *)(base + o_cF1); d.cF2 = (const double *)(base + o_cF2);
-    d.cG1 = (const double *)(base + o_cG1); d.cG2 = (const double *)(base + o_cG2);
-    d.n_bulk = (const int *)(base + o_nb); d.iS = (const int *)(base + o_iS); d.lj = (const int *)(base + o_lj);
-    d.jS_lo = (const int *)(base + o_jlo); d.jS_hi = (const int *)(base + o_jhi);
-    d.fA = (const double *)(base + o_fA); d.finvB = (const double *)(base + o_fB);
+    d.a = (const double *)(base + o_a);
+    d.binc = (const double *)(base + o_binc); d.bini = (const int2 *)(base + o_bini);
     d.band_cnt = (const int *)(base + o_cnt);
     d.band_idx = (const uint32_t *)(base + o_bidx); d.band_coef = (const double *)(base + o_bcoef);
-    d.itemsA = (const uint32_t *)(base + o_iA); d.itemsB = (const uint32_t *)(base + o_iB);
+    d.buildItems = (const uint32_t *)(base + o_bI); d.evalItems = (const uint32_t *)(base + o_eI);
+    d.dtab = (const double2 *)(base + o_dt); d.exptab = (const double *)(base + o_ex);
     b->dt = d;
     b->dev_blob = blob;
     b->device = dev;
@@ -223,6 +273,7 @@ int run(cudisc_grid g, int mode, const GasArgs &ga, StepArgs sa, cudisc_stream s
     sa.C = g->C;
     sa.Psm = g->Psm;
     sa.kslab = g->kslab;
+    sa.prof = g->prof;
     LaunchCfg lc{g->grid_ctas, g->smem_bytes, g->smem_optin};
     cudaError_t e = launch_cells(mode, lc, g->bins->dt, ga, sa, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
@@ -330,11 +381,11 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
     g->bins = b;
     g->gas_bound = false; g->fsal_valid = false;
     g->k_fsal = nullptr; g->kslab = nullptr;
-    g->stage_rho = nullptr; g->stage_err = nullptr;
+    g->stage_rho = nullptr; g->stage_err = nullptr; g->prof = nullptr;
     g->num_sms = sms; g->smem_optin = optin;
 
     const DevTables &d = b->dt;
-    const size_t vec_bytes = smem_vec_doubles(d.Np, d.partStride) * sizeof(double);
+    const size_t vec_bytes = smem_vec_doubles(d.Np, d.nchRow, d.nRng, d.nBuildItems + d.nEvalItems) * sizeof(double);
     if (vec_bytes + 16 * 64 > (size_t)optin) {
         delete g;
         return fail(CUDISC_ERR_UNSUPPORTED, "n_bins %d needs %zu B of shared memory", d.N, vec_bytes);
@@ -355,9 +406,25 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
         delete g;
         return cuda_fail(e, "cudaMalloc(grid)");
     }
+#ifdef CUDISC_PROF
+    cudaMalloc((void **)&g->prof, (size_t)g->grid_ctas * 16 * sizeof(long long));
+    cudaMemset(g->prof, 0, (size_t)g->grid_ctas * 16 * sizeof(long long));
+#endif
     *out = g;
     return CUDISC_OK;
 }
+
+#ifdef CUDISC_PROF
+/* working builds only: phase cycle counters of CTA 0..n-1, 16 per CTA; resets them */
+int cudisc_debug_prof(cudisc_grid g, long long *out_host, int n_ctas)
+{
+    cudaDeviceSynchronize();
+    n_ctas = std::min(n_ctas, g->grid_ctas);
+    cudaMemcpy(out_host, g->prof, (size_t)n_ctas * 16 * sizeof(long long), cudaMemcpyDeviceToHost);
+    cudaMemset(g->prof, 0, (size_t)g->grid_ctas * 16 * sizeof(long long));
+    return n_ctas;
+}
+#endif
 
 int cudisc_grid_bind_gas(cudisc_grid g, const cudisc_gas_state *gs)
 {
@@ -384,6 +451,7 @@ int cudisc_grid_destroy(cudisc_grid g)
     if (g->kslab) cudaFree(g->kslab);
     if (g->stage_rho) cudaFree(g->stage_rho);
     if (g->stage_err) cudaFree(g->stage_err);
+    if (g->prof) cudaFree(g->prof);
     g->magic = 0;
     delete g;
     return CUDISC_OK;

@@ -1,118 +1,358 @@
 // coag_kernels.cu -- __global__ entry points of libcudisc_coag.so (sm_100a, FP64) and their launchers.
 //
-// One persistent CTA per resident slot walks the cells c = blockIdx.x, blockIdx.x + gridDim.x, ...
+// One persistent CTA per SM walks the cells c = blockIdx.x, blockIdx.x + gridDim.x, ...
 // Every mode shares the device routines of coag_device.cuh:
 //   MODE_KERNEL : prologue + pair build                -> K_out [C][2][P] in HBM      (cudisc_coag_kernel)
 //   MODE_RATES  : K planes from HBM -> K store, eval   -> drho_dt                     (cudisc_coag_rates)
 //   MODE_OTF    : prologue + pair build -> K store, eval -> drho_dt                   (cudisc_coag_rates_otf)
 //   MODE_STEP   : prologue + pair build -> K store, BS3(2) stages (3 or 4 evals)      (cudisc_coag_step)
+// Thread k < N owns bin k: its density, stage values and derivatives live in registers.
 #include "coag_launch.h"
 
 namespace cudisc {
 
 enum { MODE_KERNEL = 0, MODE_RATES = 1, MODE_OTF = 2, MODE_STEP = 3 };
 
-template <int NT, int MODE>
-__global__ void __launch_bounds__(NT, 1)
-coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
+// ------------------------------------------------------------------------------------------ build
+// K_ij p_coag, K_ij p_frag of every pair of the cell into the K store (or, MODE_KERNEL, to HBM).
+//   rows item {c, ia, ib}: lanes <-> columns j = 32 c + lane (values of grain j stay in registers),
+//       rows i in [ia, ib), all >= 32 c + 31, two rows per iteration;
+//   list item {c, t0, t1}: pairs of diagonal block c (rows 32 c .. 32 c + 30) by triangular index
+//       t = r (r + 1) / 2 + s, i = 32 c + r, j = 32 c + s; lanes <-> t.
+template <int MODE, bool SLAB>
+__device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
+                                           const PairConst &pc, double *kout, int lane)
 {
-    extern __shared__ __align__(16) double smem_raw[];
-    const int tid = threadIdx.x;
     const int N = tb.N, P = tb.P;
-    KStore ks;
-    ks.sm = reinterpret_cast<double2 *>(smem_raw);
-    ks.Psm = sa.Psm;
-    ks.gl = reinterpret_cast<double2 *>(sa.kslab) + (size_t)blockIdx.x * (size_t)(P - sa.Psm);
-    const Smem s = carve(smem_raw + 2 * (size_t)sa.Psm, tb.Np, tb.partStride);
-    const bool has_vphi = gs.vphi != nullptr;
-    const double c15vf2 = 1.5 * gs.v_frag * gs.v_frag;
-
-    for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
-        const size_t row = (size_t)cell * N;
-
-        // ---------------- K store for this cell
-        if (MODE == MODE_RATES) {
-            const double *k0 = sa.Kin + (size_t)cell * 2 * P, *k1 = k0 + P;
-            for (int p = tid; p < P; p += NT) {
-                int i, j;
-                pair_decode(p, i, j);
-                const double h = (i == j) ? 0.5 : 1.0;
-                ks.st(p, make_double2(h * __ldg(k0 + p), h * __ldg(k1 + p)));
+    for (;;) {
+        const int it = next_item(&s.CTR[0], lane);
+        if (it >= tb.nBuildItems) break;
+        const uint32_t item = s.ITB[it];
+        const int c = (item >> 28) & 7, ia = (item >> 14) & 0x3fff, ib = item & 0x3fff;
+        if ((item >> 31) == IT_BUILD_ROWS) {
+            const int j = 32 * c + lane;
+            const bool valid = j < N;
+            const RoleJ B = load_role_j(s, valid ? j : N - 1, pc.has_vphi);
+            for (int i = ia; i < ib; i += 2) {
+                const bool two = i + 1 < ib;
+                const int i2 = two ? i + 1 : i;
+                const RoleI A1 = load_role_i(s, i, pc.has_vphi);
+                const RoleI A2 = load_role_i(s, i2, pc.has_vphi);
+                const double2 k1 = pair_kernel(A1, B, i - j, pc, s);
+                const double2 k2 = pair_kernel(A2, B, i2 - j, pc, s);
+                if (valid) {
+                    const int p1 = tri(i) + j, p2 = tri(i2) + j;
+                    if (MODE == MODE_KERNEL) {
+                        kout[p1] = k1.x; kout[P + p1] = k1.y;
+                        if (two) { kout[p2] = k2.x; kout[P + p2] = k2.y; }
+                    } else {
+                        const double h1 = (i == j) ? 0.5 : 1.0, h2 = (i2 == j) ? 0.5 : 1.0;
+                        ks.st(p1, make_double2(h1 * k1.x, h1 * k1.y));
+                        if (two) ks.st(p2, make_double2(h2 * k2.x, h2 * k2.y));
+                    }
+                }
             }
         } else {
-            const double Vg2 = cell_prologue(tb, gs, cell, s, tid);
-            __syncthreads();
-            for (int p = tid; p < P; p += NT) {
-                int i, j;
-                pair_decode(p, i, j);
-                double2 k2 = pair_kernel(s, i, j, Vg2, c15vf2, has_vphi);
+            for (int t = ia + lane; t < ib; t += 32) {
+                int r = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
+                r += (tri(r + 1) <= t) ? 1 : 0;
+                r -= (tri(r) > t) ? 1 : 0;
+                const int i = 32 * c + r, j = 32 * c + (t - tri(r));
+                const RoleI A = load_role_i(s, i, pc.has_vphi);
+                const RoleJ B = load_role_j(s, j, pc.has_vphi);
+                double2 k2 = pair_kernel(A, B, i - j, pc, s);
+                const int p = tri(i) + j;
                 if (MODE == MODE_KERNEL) {
-                    double *o = sa.out + (size_t)cell * 2 * P;
-                    o[p] = k2.x;
-                    o[P + p] = k2.y;
+                    kout[p] = k2.x; kout[P + p] = k2.y;
                 } else {
                     if (i == j) { k2.x *= 0.5; k2.y *= 0.5; }
                     ks.st(p, k2);
                 }
             }
         }
-        if (MODE == MODE_KERNEL) { __syncthreads(); continue; }
+    }
+}
 
-        // ---------------- state
-        for (int k = tid; k < N; k += NT) {
-            s.Y[k] = sa.rho[row + k];
-            if (MODE == MODE_STEP && sa.have_k1) s.K1[k] = sa.k_fsal[row + k];
+// ------------------------------------------------------------------------------------------ eval
+// One rate evaluation of the current cell: thread k < N passes y_k and gets drho_k/dt.
+// Three block barriers; every partial sum has its own slot and every combination a fixed order.
+template <int NT, bool SLAB>
+__device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
+                                             double y, int tid, long long *sa_prof)
+{
+    PROF_T(tp0);
+    const int N = tb.N, Np = tb.Np;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int k = tid;
+    const bool live = k < N;
+
+    // ---- phase 0: number densities and the (y, y m) pairs
+    double nk = 0.0;
+    if (live) {
+        nk = y * s.BINC[BC_RM * Np + k];
+        s.NN[k] = nk;
+        s.YY[k] = make_double2(y, y * s.BINC[BC_M * Np + k]);
+    }
+    if (tid == 0) s.CTR[1] = 0;
+    __syncthreads();
+    PROF_ADD(2, tp0);
+    PROF_T(tpA);
+
+    // ---- phase A: row sums, column sums and band gathers, pulled by warps
+    for (;;) {
+        const int it = next_item(&s.CTR[1], lane);
+        if (it >= tb.nEvalItems) break;
+        const uint32_t item = s.ITE[it];
+        const int kind = item >> 30, ix = (item >> 26) & 15, iy = (item >> 23) & 7;
+        const int iz = (item >> 9) & 0x1ff, iw = item & 0x1ff;
+        if (kind == IT_ROW) {
+            // lane <-> target row i of block ix, impactors j of chunk iy, j < n_bulk[i]
+            const int i = 32 * ix + lane;
+            const int jb = kRowChunk * iy;
+            int je = 0;
+            if (i < N) je = min(jb + kRowChunk, s.BINI[i].x & 0xffff);
+            const int jmax = iw;                             // max of je over the block (host)
+            const int base = tri(i);
+            double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0;
+#pragma unroll 4
+            for (int j = jb; j < jmax; ++j) {
+                if (j < je) {
+                    const double2 k2 = ks.ld(base + j);
+                    const double2 yy = s.YY[j];
+                    a1 = fma(k2.x, yy.x, a1); a2 = fma(k2.x, yy.y, a2);
+                    f1 = fma(k2.y, yy.x, f1); f2 = fma(k2.y, yy.y, f2);
+                }
+            }
+            if (i < N) {
+                double2 *pp = reinterpret_cast<double2 *>(s.PARTR + ((size_t)iy * Np + i) * 4);
+                pp[0] = make_double2(a1, a2);
+                pp[1] = make_double2(f1, f2);
+            }
+        } else if (kind == IT_COL) {
+            // lane <-> impactor column j of block ix, target rows i in [iz, iw) of range iy
+            const int j = 32 * ix + lane;
+            if (j < N) {
+                const int iSj = s.BINI[j].x >> 16;
+                double gc = 0.0, h = 0.0;
+#pragma unroll 4
+                for (int i = max(iz, j); i < iw; ++i) {
+                    const double2 k2 = ks.ld(tri(i) + j);
+                    const double ni = s.NN[i];
+                    gc = fma(k2.x, ni, gc);
+                    if (i >= iSj) h = fma(k2.y, ni, h);
+                }
+                reinterpret_cast<double2 *>(s.PARTC)[(size_t)iy * Np + j] = make_double2(gc, h);
+            }
+        } else {
+            // band gather: lane <-> target t of group ix (t < N: bins, t >= N: S bins)
+            const int t = 32 * ix + lane;
+            const int cnt = (t < 2 * N) ? __ldg(tb.band_cnt + t) : 0;
+            const int cmax = iw;
+            const uint32_t *pi = tb.band_idx + t;
+            const double *pcf = tb.band_coef + t;
+            double acc = 0.0;
+            for (int e0 = 0; e0 < cmax; e0 += 8) {
+                uint32_t ixs[8];
+                double cfs[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const bool on = e0 + u < cnt;
+                    ixs[u] = on ? __ldcg(pi + (size_t)(e0 + u) * tb.bandW) : 0u;
+                    cfs[u] = on ? __ldcg(pcf + (size_t)(e0 + u) * tb.bandW) : 0.0;
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    if (e0 + u < cnt) {
+                        const int i = ixs[u] & 0xff, j = (ixs[u] >> 8) & 0xff;
+                        const double2 k2 = ks.ld(tri(i) + j);
+                        const double kv = (ixs[u] >> 16) & 1 ? k2.y : k2.x;
+                        acc = fma(cfs[u] * s.NN[i], s.NN[j] * kv, acc);
+                    }
+                }
+            }
+            if (t < 2 * N) s.BANDV[t] = acc;
+        }
+    }
+    PROF_ADD(3, tpA);
+    __syncthreads();
+    PROF_ADD(4, tpA);
+    PROF_T(tpB);
+
+    // ---- phase B (thread <-> bin): combine partials in fixed order
+    double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, G = 0.0, sv = 0.0;
+    if (live) {
+        const int2 bi = s.BINI[k];
+        const int nch = ((bi.x & 0xffff) + kRowChunk - 1) / kRowChunk;
+        double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0;
+        for (int c = 0; c < nch; ++c) {
+            const double2 *pp = reinterpret_cast<const double2 *>(s.PARTR + ((size_t)c * Np + k) * 4);
+            const double2 u = pp[0], v = pp[1];
+            a1 += u.x; a2 += u.y; f1 += v.x; f2 += v.y;
+        }
+        const double *bc = s.BINC + k;
+        const double cA2 = bc[BC_A2 * Np], cF2 = bc[BC_F2 * Np];
+        dm1 = nk * (bc[BC_G1 * Np] * f1 - cF2 * f2);
+        d0 = nk * ((bc[BC_A1 * Np] * a1 + cA2 * a2) + (bc[BC_F1 * Np] * f1 + cF2 * f2));
+        dp1 = nk * (bc[BC_B1 * Np] * a1 - cA2 * a2);
+        // column sums of bin j over the row ranges that reach rows >= j (fixed order)
+        auto colsum = [&](int j, double &gj, double &hj) {
+            gj = 0.0; hj = 0.0;
+            for (int r = (j & ~31) / tb.rngLen; r < tb.nRng; ++r) {
+                const double2 u = reinterpret_cast<const double2 *>(s.PARTC)[(size_t)r * Np + j];
+                gj += u.x; hj += u.y;
+            }
+        };
+        double gc, h;
+        colsum(k, gc, h);
+        G = gc + h;
+        // fragment source of l-bin k, scaled by 1/B_k
+        double sl = s.BANDV[N + k];
+        for (int j = bi.y & 0xffff; j < (bi.y >> 16); ++j) {
+            double gj, hj = h;
+            if (j != k) colsum(j, gj, hj);
+            sl = fma(tb.sS * s.YY[j].x, hj, sl);
+        }
+        sv = sl * bc[BC_FIB * Np];
+    }
+    // inclusive suffix sum over bins (Eq. 67 via the l-bin algorithm): within the warp, then across
+    double suf = sv;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double v = __shfl_down_sync(0xffffffffu, suf, o);
+        if (lane + o < 32) suf += v;
+    }
+    double *wtot = s.RED, *eUp = s.RED + 16, *eDn = s.RED + 32;
+    if (lane == 0) { wtot[warp] = suf; eDn[warp] = dm1; }
+    if (lane == 31) eUp[warp] = dp1;
+    const double up = __shfl_up_sync(0xffffffffu, dp1, 1);
+    const double dn = __shfl_down_sync(0xffffffffu, dm1, 1);
+    __syncthreads();
+
+    double d = 0.0;
+    if (live) {
+        const int nw = (N + 31) >> 5;
+        for (int w = warp + 1; w < nw; ++w) suf += wtot[w];
+        const double prev = (lane > 0) ? up : (warp > 0 ? eUp[warp - 1] : 0.0);
+        const double next = (lane < 31) ? dn : (warp + 1 < nw ? eDn[warp + 1] : 0.0);
+        d = d0;
+        if (k > 0) d += prev;
+        if (k < N - 1) d += next;
+        d += s.BANDV[k];
+        d = fma(-y, G, d);
+        d = fma(s.BINC[BC_FA * Np + k], suf, d);
+    }
+    PROF_ADD(5, tpB);
+    return d;
+}
+
+template <int NT, int MODE, bool SLAB>
+__global__ void __launch_bounds__(NT, 1)
+coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
+{
+    extern __shared__ __align__(16) double smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int N = tb.N, P = tb.P;
+    KStore<SLAB> ks;
+    ks.sm = reinterpret_cast<double2 *>(smem_raw);
+    ks.Psm = sa.Psm;
+    ks.gl = reinterpret_cast<double2 *>(sa.kslab) + (size_t)blockIdx.x * (size_t)(P - sa.Psm);
+    const Smem s = carve(smem_raw + 2 * (size_t)sa.Psm, tb.Np, tb.nchRow, tb.nRng, tb.nBuildItems,
+                         tb.nEvalItems);
+    PairConst pc;
+    pc.has_vphi = gs.vphi != nullptr;
+    pc.logGrid = tb.logGrid != 0;
+    pc.c15vf2 = 1.5 * gs.v_frag * gs.v_frag;
+    pc.Vg2 = 0.0;
+
+    // per-CTA constants in shared memory
+    for (int q = tid; q < 64; q += NT) s.EXPT[q] = tb.exptab[q];
+    if (tb.logGrid) for (int q = tid; q < N; q += NT) s.DTAB[q] = tb.dtab[q];
+    for (int q = tid; q < kBinC * tb.Np; q += NT) s.BINC[q] = tb.binc[q];
+    for (int q = tid; q < N; q += NT) s.BINI[q] = tb.bini[q];
+    for (int q = tid; q < tb.nBuildItems; q += NT) s.ITB[q] = tb.buildItems[q];
+    for (int q = tid; q < tb.nEvalItems; q += NT) s.ITE[q] = tb.evalItems[q];
+    __syncthreads();
+
+    long long *sa_prof = sa.prof ? sa.prof + 16 * (size_t)blockIdx.x : nullptr;
+    (void)sa_prof;
+    for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
+        PROF_T(tc0);
+        const size_t row = (size_t)cell * N;
+        const int k = tid;
+        const bool live = k < N;
+
+        // ---------------- K store for this cell
+        if (MODE == MODE_RATES) {
+            const double *k0 = sa.Kin + (size_t)cell * 2 * P, *k1 = k0 + P;
+            for (int i = tid >> 5; i < N; i += NT / 32) {
+                const int base = tri(i);
+                for (int j = lane; j <= i; j += 32) {
+                    const double h = (i == j) ? 0.5 : 1.0;
+                    ks.st(base + j, make_double2(h * __ldg(k0 + base + j), h * __ldg(k1 + base + j)));
+                }
+            }
+        } else {
+            pc.Vg2 = cell_prologue(tb, gs, cell, s, tid, NT);
+            if (tid == 0) s.CTR[0] = 0;
+            __syncthreads();
+            PROF_ADD(0, tc0);
+            build_cell<MODE, SLAB>(tb, s, ks, pc, MODE == MODE_KERNEL ? sa.out + (size_t)cell * 2 * P : nullptr, lane);
         }
         __syncthreads();
+        PROF_ADD(1, tc0);
+        if (MODE == MODE_KERNEL) continue;
+
+        // ---------------- state (thread <-> bin)
+        const double y0 = live ? sa.rho[row + k] : 0.0;
 
         if (MODE == MODE_RATES || MODE == MODE_OTF) {
-            eval_rates<NT>(tb, s, ks, s.Y, s.K1, tid);
-            for (int k = tid; k < N; k += NT) sa.out[row + k] = s.K1[k];
+            const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, sa_prof);
+            if (live) sa.out[row + k] = d;
             __syncthreads();
             continue;
         }
 
         // ---------------- Bogacki-Shampine 3(2), PAPER.md:478 (tableau: Bogacki & Shampine 1989)
         const double h = sa.dt;
-        if (!sa.have_k1) eval_rates<NT>(tb, s, ks, s.Y, s.K1, tid);
-        for (int k = tid; k < N; k += NT) s.YS[k] = s.Y[k] + 0.5 * h * s.K1[k];
-        __syncthreads();
-        eval_rates<NT>(tb, s, ks, s.YS, s.K2, tid);
-        for (int k = tid; k < N; k += NT) s.YS[k] = s.Y[k] + 0.75 * h * s.K2[k];
-        __syncthreads();
-        eval_rates<NT>(tb, s, ks, s.YS, s.K3, tid);
-        for (int k = tid; k < N; k += NT)
-            s.YS[k] = s.Y[k] + h * ((2.0 / 9.0) * s.K1[k] + (1.0 / 3.0) * s.K2[k] + (4.0 / 9.0) * s.K3[k]);
-        __syncthreads();
-        eval_rates<NT>(tb, s, ks, s.YS, s.K4, tid);
+        double k1 = 0.0, k2 = 0.0, k3 = 0.0, k4 = 0.0, yn = y0;
+        if (sa.have_k1) k1 = live ? sa.k_fsal[row + k] : 0.0;
+#pragma unroll 1
+        for (int st = sa.have_k1 ? 1 : 0; st < 4; ++st) {
+            double ys = y0;
+            if (st == 1) ys = y0 + 0.5 * h * k1;
+            if (st == 2) ys = y0 + 0.75 * h * k2;
+            if (st == 3) { yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3); ys = yn; }
+            const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, sa_prof);
+            if (st == 0) k1 = d;
+            if (st == 1) k2 = d;
+            if (st == 2) k3 = d;
+            if (st == 3) k4 = d;
+        }
 
         // error norm (R10) and write-back
-        double part = 0.0;
-        for (int k = tid; k < N; k += NT) part += s.Y[k];
-        const double atol = sa.atol_factor * block_sum<NT>(part, s.RED, tid);
+        const double atol = sa.atol_factor * block_sum<NT>(y0, s.RED + 48, tid);
         double emax = 0.0;
-        for (int k = tid; k < N; k += NT) {
-            const double e = h * ((-5.0 / 72.0) * s.K1[k] + (1.0 / 12.0) * s.K2[k]
-                                  + (1.0 / 9.0) * s.K3[k] - (1.0 / 8.0) * s.K4[k]);
-            const double sc = atol + sa.rtol * fmax(fabs(s.Y[k]), fabs(s.YS[k]));
-            emax = nanmax(emax, fabs(e) / sc);
-            sa.rho_out[row + k] = s.YS[k];
-            sa.k_out[row + k] = s.K4[k];
+        if (live) {
+            const double e = h * ((-5.0 / 72.0) * k1 + (1.0 / 12.0) * k2 + (1.0 / 9.0) * k3 - (1.0 / 8.0) * k4);
+            const double sc = atol + sa.rtol * fmax(fabs(y0), fabs(yn));
+            emax = fabs(e) / sc;
+            sa.rho_out[row + k] = yn;
+            sa.k_out[row + k] = k4;
         }
-        emax = block_nanmax<NT>(emax, s.RED, tid);
+        emax = block_nanmax<NT>(emax, s.RED + 48, tid);
         if (tid == 0) sa.err[cell] = emax;
-        __syncthreads();
+        PROF_ADD(6, tc0);
     }
 }
 
 // ------------------------------------------------------------------------------------------ launch
-template <int MODE>
+template <int MODE, bool SLAB>
 static cudaError_t launch_mode(const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
                                const StepArgs &sa, cudaStream_t st)
 {
     constexpr int NT = kThreads;
-    auto fn = coag_cells_kernel<NT, MODE>;
-    static bool attr_done = false;          // per process and per mode; same value every time
+    auto fn = coag_cells_kernel<NT, MODE, SLAB>;
+    static bool attr_done = false;          // per process and per instantiation; same value every time
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              lc.smem_optin);
@@ -123,20 +363,29 @@ static cudaError_t launch_mode(const LaunchCfg &lc, const DevTables &tb, const G
     return cudaGetLastError();
 }
 
+template <bool SLAB>
+static cudaError_t launch_slab(int mode, const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
+                               const StepArgs &sa, cudaStream_t st)
+{
+    switch (mode) {
+    case MODE_KERNEL: return launch_mode<MODE_KERNEL, SLAB>(lc, tb, gs, sa, st);
+    case MODE_RATES: return launch_mode<MODE_RATES, SLAB>(lc, tb, gs, sa, st);
+    case MODE_OTF: return launch_mode<MODE_OTF, SLAB>(lc, tb, gs, sa, st);
+    default: return launch_mode<MODE_STEP, SLAB>(lc, tb, gs, sa, st);
+    }
+}
+
 cudaError_t launch_cells(int mode, const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
                          const StepArgs &sa, cudaStream_t st)
 {
-    switch (mode) {
-    case MODE_KERNEL: return launch_mode<MODE_KERNEL>(lc, tb, gs, sa, st);
-    case MODE_RATES: return launch_mode<MODE_RATES>(lc, tb, gs, sa, st);
-    case MODE_OTF: return launch_mode<MODE_OTF>(lc, tb, gs, sa, st);
-    default: return launch_mode<MODE_STEP>(lc, tb, gs, sa, st);
-    }
+    // SLAB: part of the K store lives in the per-CTA global slab (n_bins too large for shared memory)
+    return sa.Psm < tb.P ? launch_slab<true>(mode, lc, tb, gs, sa, st)
+                         : launch_slab<false>(mode, lc, tb, gs, sa, st);
 }
 
 int cells_occupancy(int smem_bytes, int smem_optin)
 {
-    auto fn = coag_cells_kernel<kThreads, MODE_STEP>;
+    auto fn = coag_cells_kernel<kThreads, MODE_STEP, true>;
     if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
         return 0;
     int n = 0;
