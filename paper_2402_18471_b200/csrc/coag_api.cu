@@ -207,11 +207,17 @@ int upload_tables(cudisc_bins b)
         bcoef[(size_t)e2 * W + be.target] = be.coef;
     }
     d.bandW = W; d.bandL = L;
+    // band tables in tensor memory when they fit: warp g of the CTA owns target group g
+    const int nGroups = (2 * N + 31) / 32;
+    d.bandLp = (L + 7) & ~7;
+    d.bandTmem = (d.bandLp <= kBandTmemMax && nGroups <= kThreads / 32) ? 1 : 0;
+    std::vector<int> bandGrp(16, 0);
     std::vector<uint32_t> evalItems;
-    for (int tg = 0; tg * 32 < 2 * N; ++tg) {
+    for (int tg = 0; tg < nGroups; ++tg) {
         int cmax = 0;
         for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
-        evalItems.push_back(pack_eval(IT_BAND, tg, 0, 0, cmax));
+        if (tg < 16) bandGrp[tg] = (cmax + 7) & ~7;
+        if (!d.bandTmem) evalItems.push_back(pack_eval(IT_BAND, tg, 0, 0, cmax));
     }
     for (const Cost &c : work) evalItems.push_back(c.item);
     d.nBuildItems = (int)buildItems.size(); d.nEvalItems = (int)evalItems.size();
@@ -220,7 +226,7 @@ int upload_tables(cudisc_bins b)
     const size_t o_a = bl.add(t.a), o_binc = bl.add(binc), o_bini = bl.add(bini);
     const size_t o_cnt = bl.add(cnt), o_bidx = bl.add(bidx), o_bcoef = bl.add(bcoef);
     const size_t o_bI = bl.add(buildItems), o_eI = bl.add(evalItems);
-    const size_t o_dt = bl.add(dtab), o_ex = bl.add(exptab);
+    const size_t o_dt = bl.add(dtab), o_ex = bl.add(exptab), o_bg = bl.add(bandGrp);
 
     void *blob = nullptr;
     e = cudaMalloc(&blob, bl.bytes.size());
@@ -234,6 +240,7 @@ int upload_tables(cudisc_bins b)
     d.band_idx = (const uint32_t *)(base + o_bidx); d.band_coef = (const double *)(base + o_bcoef);
     d.buildItems = (const uint32_t *)(base + o_bI); d.evalItems = (const uint32_t *)(base + o_eI);
     d.dtab = (const double2 *)(base + o_dt); d.exptab = (const double *)(base + o_ex);
+    d.band_grp = (const int *)(base + o_bg);
     b->dt = d;
     b->dev_blob = blob;
     b->device = dev;

@@ -78,7 +78,7 @@ __device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, c
 // Three block barriers; every partial sum has its own slot and every combination a fixed order.
 template <int NT, bool SLAB>
 __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
-                                             double y, int tid, long long *sa_prof)
+                                             double y, int tid, uint32_t tbase, long long *sa_prof)
 {
     PROF_T(tp0);
     const int N = tb.N, Np = tb.Np;
@@ -98,7 +98,30 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     PROF_ADD(2, tp0);
     PROF_T(tpA);
 
-    // ---- phase A: row sums, column sums and band gathers, pulled by warps
+    // ---- phase A: band gather from tensor memory (warp g <-> target group g), then row sums,
+    //      column sums (and, without tensor-memory tables, band gathers) pulled by warps
+    if (tb.bandTmem && 32 * warp < 2 * N) {
+        const int t = 32 * warp + lane;
+        const int Lg = s.CTR[4 + warp], Lp = tb.bandLp;
+        const uint32_t tc = tmem_warp_addr(tbase, warp, 0), ti = tc + 2 * Lp;
+        const double *kd = reinterpret_cast<const double *>(ks.sm);
+        double acc = 0.0;
+        for (int e0 = 0; e0 < Lg; e0 += 8) {
+            uint32_t cf[16], ixs[8];
+            tmem_ld16(tc + 2 * e0, cf);
+            tmem_ld8(ti + e0, ixs);
+            tmem_wait_ld();
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int i = ixs[u] & 0xff, j = (ixs[u] >> 8) & 0xff;
+                const int p2 = 2 * (tri(i) + j) + (int)((ixs[u] >> 16) & 1);
+                const double kv = SLAB ? ((ixs[u] >> 16) & 1 ? ks.ld(p2 >> 1).y : ks.ld(p2 >> 1).x) : kd[p2];
+                const double c = __hiloint2double((int)cf[2 * u + 1], (int)cf[2 * u]);
+                acc = fma(c * s.NN[i], s.NN[j] * kv, acc);
+            }
+        }
+        if (t < 2 * N) s.BANDV[t] = acc;
+    }
     for (;;) {
         const int it = next_item(&s.CTR[1], lane);
         if (it >= tb.nEvalItems) break;
@@ -271,7 +294,50 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
     for (int q = tid; q < N; q += NT) s.BINI[q] = tb.bini[q];
     for (int q = tid; q < tb.nBuildItems; q += NT) s.ITB[q] = tb.buildItems[q];
     for (int q = tid; q < tb.nEvalItems; q += NT) s.ITE[q] = tb.evalItems[q];
+    if (tid < 16) s.CTR[4 + tid] = tb.band_grp[tid];
+    // band tables -> tensor memory (grid-only constants, once per CTA)
+    uint32_t tbase = 0;
+    const bool use_tmem = MODE != MODE_KERNEL && tb.bandTmem;
+    if (use_tmem) {
+        uint32_t *slot = reinterpret_cast<uint32_t *>(s.RED);
+        if (tid < 32) tmem_alloc_all(slot);
+        tmem_fence_before();
+        __syncthreads();
+        tmem_fence_after();
+        tbase = *slot;
+        const int warp = tid >> 5;
+        if (32 * warp < 2 * N) {
+            const int t = 32 * warp + lane, Lp = tb.bandLp;
+            const int cnt = tb.band_cnt[t];                        // band_cnt is padded to bandW >= 32 groups
+            for (int e0 = 0; e0 < Lp; e0 += 8) {
+                uint32_t v[8];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int e = e0 + u;
+                    const double c = e < cnt ? tb.band_coef[(size_t)e * tb.bandW + t] : 0.0;
+                    v[2 * u] = (uint32_t)__double2loint(c); v[2 * u + 1] = (uint32_t)__double2hiint(c);
+                }
+                tmem_st8(tmem_warp_addr(tbase, warp, 2 * e0), v);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int e = e0 + 4 + u;
+                    const double c = e < cnt ? tb.band_coef[(size_t)e * tb.bandW + t] : 0.0;
+                    v[2 * u] = (uint32_t)__double2loint(c); v[2 * u + 1] = (uint32_t)__double2hiint(c);
+                }
+                tmem_st8(tmem_warp_addr(tbase, warp, 2 * e0 + 8), v);
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int e = e0 + u;
+                    v[u] = e < cnt ? tb.band_idx[(size_t)e * tb.bandW + t] : 0u;
+                }
+                tmem_st8(tmem_warp_addr(tbase, warp, 2 * Lp + e0), v);
+            }
+            tmem_wait_st();
+        }
+        tmem_fence_before();
+    }
     __syncthreads();
+    if (use_tmem) tmem_fence_after();
 
     long long *sa_prof = sa.prof ? sa.prof + 16 * (size_t)blockIdx.x : nullptr;
     (void)sa_prof;
@@ -306,7 +372,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
         const double y0 = live ? sa.rho[row + k] : 0.0;
 
         if (MODE == MODE_RATES || MODE == MODE_OTF) {
-            const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, sa_prof);
+            const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, tbase, sa_prof);
             if (live) sa.out[row + k] = d;
             __syncthreads();
             continue;
@@ -322,7 +388,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
             if (st == 1) ys = y0 + 0.5 * h * k1;
             if (st == 2) ys = y0 + 0.75 * h * k2;
             if (st == 3) { yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3); ys = yn; }
-            const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, sa_prof);
+            const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, tbase, sa_prof);
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;
             if (st == 2) k3 = d;
@@ -342,6 +408,11 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
         emax = block_nanmax<NT>(emax, s.RED + 48, tid);
         if (tid == 0) sa.err[cell] = emax;
         PROF_ADD(6, tc0);
+    }
+    if (use_tmem) {
+        tmem_fence_before();
+        __syncthreads();
+        if (tid < 32) tmem_dealloc_all(tbase);
     }
 }
 
