@@ -130,10 +130,10 @@ int upload_tables(cudisc_bins b)
     std::vector<uint32_t> buildItems;
     constexpr int kRowsPerItem = 4, kPairsPerItem = 64;
     for (int c = 0; c < nblk; ++c)
-        for (int ia = 32 * c + 31; ia < N; ia += kRowsPerItem)
+        for (int ia = 32 * c + 32; ia < N; ia += kRowsPerItem)
             buildItems.push_back(pack_build(IT_BUILD_ROWS, c, ia, std::min(N, ia + kRowsPerItem)));
     for (int c = 0; c < nblk; ++c) {
-        const int rows = std::min(32 * c + 31, N) - 32 * c;          // rows 32 c .. 32 c + rows - 1
+        const int rows = std::min(32 * c + 32, N) - 32 * c;          // rows 32 c .. 32 c + rows - 1
         const int last = rows * (rows + 1) / 2;
         for (int a = 0; a < last; a += kPairsPerItem)
             buildItems.push_back(pack_build(IT_BUILD_LIST, c, a, std::min(last, a + kPairsPerItem)));

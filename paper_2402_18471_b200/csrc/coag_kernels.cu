@@ -16,12 +16,13 @@ enum { MODE_KERNEL = 0, MODE_RATES = 1, MODE_OTF = 2, MODE_STEP = 3 };
 // ------------------------------------------------------------------------------------------ build
 // K_ij p_coag, K_ij p_frag of every pair of the cell into the K store (or, MODE_KERNEL, to HBM).
 //   rows item {c, ia, ib}: lanes <-> columns j = 32 c + lane (values of grain j stay in registers),
-//       rows i in [ia, ib), all >= 32 c + 31, two rows per iteration;
-//   list item {c, t0, t1}: pairs of diagonal block c (rows 32 c .. 32 c + 30) by triangular index
+//       rows i in [ia, ib), all >= 32 c + 32 (no diagonal pair), two rows per iteration (an odd last
+//       row is computed twice);
+//   list item {c, t0, t1}: pairs of diagonal block c (rows 32 c .. 32 c + 31) by triangular index
 //       t = r (r + 1) / 2 + s, i = 32 c + r, j = 32 c + s; lanes <-> t.
-template <int MODE, bool SLAB>
-__device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
-                                           const PairConst &pc, double *kout, int lane)
+template <int MODE, bool SLAB, bool VPHI, bool LOG>
+__device__ __forceinline__ void build_items(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
+                                            const PairConst &pc, double *kout, int lane)
 {
     const int N = tb.N, P = tb.P;
     for (;;) {
@@ -32,23 +33,21 @@ __device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, c
         if ((item >> 31) == IT_BUILD_ROWS) {
             const int j = 32 * c + lane;
             const bool valid = j < N;
-            const RoleJ B = load_role_j(s, valid ? j : N - 1, pc.has_vphi);
+            const RoleJ B = load_role_j<VPHI>(s, valid ? j : N - 1);
             for (int i = ia; i < ib; i += 2) {
-                const bool two = i + 1 < ib;
-                const int i2 = two ? i + 1 : i;
-                const RoleI A1 = load_role_i(s, i, pc.has_vphi);
-                const RoleI A2 = load_role_i(s, i2, pc.has_vphi);
-                const double2 k1 = pair_kernel(A1, B, i - j, pc, s);
-                const double2 k2 = pair_kernel(A2, B, i2 - j, pc, s);
+                const int i2 = min(i + 1, ib - 1);
+                const RoleI A1 = load_role_i<VPHI>(s, i);
+                const RoleI A2 = load_role_i<VPHI>(s, i2);
+                const double2 k1 = pair_kernel<VPHI, LOG>(A1, B, i - j, pc, s);
+                const double2 k2 = pair_kernel<VPHI, LOG>(A2, B, i2 - j, pc, s);
                 if (valid) {
                     const int p1 = tri(i) + j, p2 = tri(i2) + j;
                     if (MODE == MODE_KERNEL) {
                         kout[p1] = k1.x; kout[P + p1] = k1.y;
-                        if (two) { kout[p2] = k2.x; kout[P + p2] = k2.y; }
+                        kout[p2] = k2.x; kout[P + p2] = k2.y;
                     } else {
-                        const double h1 = (i == j) ? 0.5 : 1.0, h2 = (i2 == j) ? 0.5 : 1.0;
-                        ks.st(p1, make_double2(h1 * k1.x, h1 * k1.y));
-                        if (two) ks.st(p2, make_double2(h2 * k2.x, h2 * k2.y));
+                        ks.st(p1, k1);
+                        ks.st(p2, k2);
                     }
                 }
             }
@@ -58,9 +57,9 @@ __device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, c
                 r += (tri(r + 1) <= t) ? 1 : 0;
                 r -= (tri(r) > t) ? 1 : 0;
                 const int i = 32 * c + r, j = 32 * c + (t - tri(r));
-                const RoleI A = load_role_i(s, i, pc.has_vphi);
-                const RoleJ B = load_role_j(s, j, pc.has_vphi);
-                double2 k2 = pair_kernel(A, B, i - j, pc, s);
+                const RoleI A = load_role_i<VPHI>(s, i);
+                const RoleJ B = load_role_j<VPHI>(s, j);
+                double2 k2 = pair_kernel<VPHI, LOG>(A, B, i - j, pc, s);
                 const int p = tri(i) + j;
                 if (MODE == MODE_KERNEL) {
                     kout[p] = k2.x; kout[P + p] = k2.y;
@@ -70,6 +69,20 @@ __device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, c
                 }
             }
         }
+    }
+}
+
+template <int MODE, bool SLAB>
+__device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
+                                           const PairConst &pc, bool has_vphi, double *kout, int lane)
+{
+    // warp-uniform dispatch: the inner loops are compiled for their case
+    if (has_vphi) {
+        if (tb.logGrid) build_items<MODE, SLAB, true, true>(tb, s, ks, pc, kout, lane);
+        else build_items<MODE, SLAB, true, false>(tb, s, ks, pc, kout, lane);
+    } else {
+        if (tb.logGrid) build_items<MODE, SLAB, false, true>(tb, s, ks, pc, kout, lane);
+        else build_items<MODE, SLAB, false, false>(tb, s, ks, pc, kout, lane);
     }
 }
 
@@ -282,8 +295,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
     const Smem s = carve(smem_raw + 2 * (size_t)sa.Psm, tb.Np, tb.nchRow, tb.nRng, tb.nBuildItems,
                          tb.nEvalItems);
     PairConst pc;
-    pc.has_vphi = gs.vphi != nullptr;
-    pc.logGrid = tb.logGrid != 0;
+    const bool has_vphi = gs.vphi != nullptr;
     pc.c15vf2 = 1.5 * gs.v_frag * gs.v_frag;
     pc.Vg2 = 0.0;
 
@@ -341,11 +353,28 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
 
     long long *sa_prof = sa.prof ? sa.prof + 16 * (size_t)blockIdx.x : nullptr;
     (void)sa_prof;
+    const int k = tid;
+    const bool live = k < N;
+
+    // frozen inputs of a cell, fetched one cell ahead: the loads of cell c + grid
+    // are issued before the last rate evaluation of cell c
+    CellGas nx = {1.0, 1.0, 1.0, 1.0};
+    double nvR = 0.0, nvZ = 0.0, nvP = 0.0;
+    auto fetch = [&](int cell) {
+        if (MODE == MODE_RATES || cell >= sa.C) return;
+        nx.T = __ldg(gs.T + cell); nx.rho_g = __ldg(gs.rho_g + cell); nx.Om = __ldg(gs.Omega + cell);
+        nx.alpha = gs.alpha ? __ldg(gs.alpha + cell) : gs.alpha_const;
+        if (live) {
+            const size_t g = (size_t)cell * N + k;
+            nvR = __ldg(gs.vR + g); nvZ = __ldg(gs.vZ + g);
+            if (has_vphi) nvP = __ldg(gs.vphi + g);
+        }
+    };
+    fetch(blockIdx.x);
+
     for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
         PROF_T(tc0);
         const size_t row = (size_t)cell * N;
-        const int k = tid;
-        const bool live = k < N;
 
         // ---------------- K store for this cell
         if (MODE == MODE_RATES) {
@@ -358,20 +387,27 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
                 }
             }
         } else {
-            pc.Vg2 = cell_prologue(tb, gs, cell, s, tid, NT);
+            pc.Vg2 = cell_prologue(tb, nx, gs.mu, gs.sigma_mol, nvR, nvZ, nvP, has_vphi, s, k);
             if (tid == 0) s.CTR[0] = 0;
             __syncthreads();
             PROF_ADD(0, tc0);
-            build_cell<MODE, SLAB>(tb, s, ks, pc, MODE == MODE_KERNEL ? sa.out + (size_t)cell * 2 * P : nullptr, lane);
         }
+        // state (thread <-> bin): in flight during the build
+        double y0 = 0.0, k1 = 0.0;
+        if (MODE != MODE_KERNEL && live) {
+            y0 = sa.rho[row + k];
+            if (MODE == MODE_STEP && sa.have_k1) k1 = sa.k_fsal[row + k];
+        }
+        if (MODE != MODE_RATES)
+            build_cell<MODE, SLAB>(tb, s, ks, pc, has_vphi,
+                                   MODE == MODE_KERNEL ? sa.out + (size_t)cell * 2 * P : nullptr, lane);
+        if (MODE == MODE_KERNEL) fetch(cell + gridDim.x);
         __syncthreads();
         PROF_ADD(1, tc0);
         if (MODE == MODE_KERNEL) continue;
 
-        // ---------------- state (thread <-> bin)
-        const double y0 = live ? sa.rho[row + k] : 0.0;
-
         if (MODE == MODE_RATES || MODE == MODE_OTF) {
+            fetch(cell + gridDim.x);
             const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, tbase, sa_prof);
             if (live) sa.out[row + k] = d;
             __syncthreads();
@@ -380,14 +416,17 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
 
         // ---------------- Bogacki-Shampine 3(2), PAPER.md:478 (tableau: Bogacki & Shampine 1989)
         const double h = sa.dt;
-        double k1 = 0.0, k2 = 0.0, k3 = 0.0, k4 = 0.0, yn = y0;
-        if (sa.have_k1) k1 = live ? sa.k_fsal[row + k] : 0.0;
+        double k2 = 0.0, k3 = 0.0, k4 = 0.0, yn = y0;
 #pragma unroll 1
         for (int st = sa.have_k1 ? 1 : 0; st < 4; ++st) {
             double ys = y0;
             if (st == 1) ys = y0 + 0.5 * h * k1;
             if (st == 2) ys = y0 + 0.75 * h * k2;
-            if (st == 3) { yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3); ys = yn; }
+            if (st == 3) {
+                yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
+                ys = yn;
+                fetch(cell + gridDim.x);
+            }
             const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, tbase, sa_prof);
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;
