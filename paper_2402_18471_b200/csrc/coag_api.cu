@@ -139,10 +139,26 @@ int upload_tables(cudisc_bins b)
             buildItems.push_back(pack_build(IT_BUILD_LIST, c, a, std::min(last, a + kPairsPerItem)));
     }
 
-    // ---- eval items: band gathers first (global-memory latency), then row / column passes by cost
-    const int nchRow = std::max(1, (N + kRowChunk - 1) / kRowChunk);
-    const int nRng = std::max(1, (N + 63) / 64);
+    // ---- eval items: row / column passes, heaviest first.  Partial sums go to packed slots:
+    //      row chunk c holds rows i >= rowFirst[c], column range r holds columns j < R1[r]
+    const int nchRow = std::min(8, std::max(1, (N + kRowChunk - 1) / kRowChunk));
+    const int nRng = std::min(8, std::max(1, (N + 31) / 32));
     const int rngLen = (N + nRng - 1) / nRng;
+    std::vector<int> sched(kSched, 0);
+    int rowSlots = 0, colSlots = 0;
+    for (int c = 0; c < nchRow; ++c) {
+        int first = N;
+        for (int i = 0; i < N; ++i)
+            if (t.n_bulk[i] > kRowChunk * c) { first = i; break; }
+        sched[SC_ROWFIRST + c] = first;
+        sched[SC_ROWOFF + c] = rowSlots;
+        rowSlots += N - first;
+    }
+    for (int r = 0; r < nRng; ++r) {
+        sched[SC_COLOFF + r] = colSlots;
+        colSlots += std::min(N, (r + 1) * rngLen);
+    }
+    d.partRowSlots = rowSlots; d.partColSlots = colSlots;
     struct Cost { uint32_t item; long cost; };
     std::vector<Cost> work;
     for (int blk = 0; blk < nblk; ++blk)
@@ -150,14 +166,16 @@ int upload_tables(cudisc_bins b)
             int jmax = 0;
             for (int i = blk * 32; i < std::min(N, blk * 32 + 32); ++i)
                 jmax = std::max(jmax, std::min(kRowChunk * cw + kRowChunk, t.n_bulk[i]));
-            if (jmax <= kRowChunk * cw) continue;
-            work.push_back({pack_eval(IT_ROW, blk, cw, 0, jmax), 5L * (jmax - kRowChunk * cw)});
+            // the item must exist (and write zeros) whenever a row of the block owns a slot of chunk cw
+            if (std::min(N, blk * 32 + 32) <= sched[SC_ROWFIRST + cw]) continue;
+            jmax = std::max(jmax, kRowChunk * cw);
+            work.push_back({pack_eval(IT_ROW, blk, cw, 0, jmax), 5L * (jmax - kRowChunk * cw) + 20});
         }
     for (int cb = 0; cb < nblk; ++cb)
         for (int r = 0; r < nRng; ++r) {
             const int i0 = r * rngLen, i1 = std::min(N, (r + 1) * rngLen);
             if (i1 <= 32 * cb) continue;
-            work.push_back({pack_eval(IT_COL, cb, r, i0, i1), 5L * (i1 - std::max(i0, 32 * cb))});
+            work.push_back({pack_eval(IT_COL, cb, r, i0, i1), 5L * (i1 - std::max(i0, 32 * cb)) + 20});
         }
     std::stable_sort(work.begin(), work.end(), [](const Cost &x, const Cost &y) { return x.cost > y.cost; });
     d.nchRow = nchRow; d.nRng = nRng; d.rngLen = rngLen;
@@ -172,7 +190,9 @@ int upload_tables(cudisc_bins b)
         binc[(size_t)BC_F1 * d.Np + k] = t.cF1[k]; binc[(size_t)BC_F2 * d.Np + k] = t.cF2[k];
         binc[(size_t)BC_G1 * d.Np + k] = t.cG1[k];
         binc[(size_t)BC_FA * d.Np + k] = t.fA[k];  binc[(size_t)BC_FIB * d.Np + k] = t.finvB[k];
-        bini[k] = make_int2(t.n_bulk[k] | (t.iS[k] << 16), t.jS_lo[k] | (t.jS_hi[k] << 16));
+        // n_bulk <= 256 and iS <= 256 need 9 bits each; first column range r with R1[r] > k
+        bini[k] = make_int2(t.n_bulk[k] | (t.iS[k] << 9) | ((k / rngLen) << 18),
+                            t.jS_lo[k] | (t.jS_hi[k] << 16));
     }
 
     // per-offset tables of a log grid: sigma_ij = a_i^2 pi (1 + q^-d)^2, (St_i - St_j)/(St_i + St_j)
@@ -207,17 +227,52 @@ int upload_tables(cudisc_bins b)
         bcoef[(size_t)e2 * W + be.target] = be.coef;
     }
     d.bandW = W; d.bandL = L;
-    // band tables in tensor memory when they fit: warp g of the CTA owns target group g
+    // band tables in tensor memory when they fit: target group g sits in the tensor-memory lanes of
+    // quarter g % 4 (columns 128 (g / 4) ...), readable by warps w with w % 4 == g % 4.  Its entry
+    // list is cut into tasks of <= kBandTask entries, dealt to the least loaded warp of the quarter;
+    // a group cut in two sums into the two BANDV slots.
     const int nGroups = (2 * N + 31) / 32;
     d.bandLp = (L + 7) & ~7;
     d.bandTmem = (d.bandLp <= kBandTmemMax && nGroups <= kThreads / 32) ? 1 : 0;
-    std::vector<int> bandGrp(16, 0);
     std::vector<uint32_t> evalItems;
-    for (int tg = 0; tg < nGroups; ++tg) {
-        int cmax = 0;
-        for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
-        if (tg < 16) bandGrp[tg] = (cmax + 7) & ~7;
-        if (!d.bandTmem) evalItems.push_back(pack_eval(IT_BAND, tg, 0, 0, cmax));
+    {
+        constexpr int nWarps = kThreads / 32;
+        int load[nWarps] = {0}, ntask[nWarps] = {0};
+        for (int tg = 0; tg < nGroups; ++tg) {
+            int cmax = 0;
+            for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
+            if (!d.bandTmem) { evalItems.push_back(pack_eval(IT_BAND, tg, 0, 0, cmax)); continue; }
+            const int Lg = (cmax + 7) & ~7;
+            if (Lg == 0) continue;   // phase 0 does not zero slot 0: every group with targets needs a task
+        }
+        if (d.bandTmem) {
+            for (int tg = 0; tg < nGroups; ++tg) {
+                int cmax = 0;
+                for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
+                const int Lg = (cmax + 7) & ~7;
+                const int half = (Lg > 16) ? ((Lg / 2 + 7) & ~7) : Lg;
+                const int cuts[3] = {0, half, Lg};
+                for (int h = 0; h < 2; ++h) {
+                    if (h == 1 && cuts[1] == cuts[2]) break;
+                    int best = -1;
+                    for (int w = tg % 4; w < nWarps; w += 4)
+                        if (ntask[w] < 2 && (best < 0 || load[w] < load[best])) best = w;
+                    if (best < 0) { d.bandTmem = 0; break; }
+                    sched[SC_BTASK + 2 * best + ntask[best]] =
+                        (int)(0x80000000u | ((uint32_t)h << 30) | ((uint32_t)tg << 16) |
+                              ((uint32_t)cuts[h] << 8) | (uint32_t)cuts[h + 1]);
+                    ntask[best]++;
+                    load[best] += cuts[h + 1] - cuts[h] + 4;
+                }
+            }
+        }
+        if (!d.bandTmem && evalItems.empty())
+            for (int tg = 0; tg < nGroups; ++tg) {
+                int cmax = 0;
+                for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
+                evalItems.push_back(pack_eval(IT_BAND, tg, 0, 0, cmax));
+            }
+        if (!d.bandTmem) for (int q = 0; q < 2 * nWarps; ++q) sched[SC_BTASK + q] = 0;
     }
     for (const Cost &c : work) evalItems.push_back(c.item);
     d.nBuildItems = (int)buildItems.size(); d.nEvalItems = (int)evalItems.size();
@@ -226,7 +281,7 @@ int upload_tables(cudisc_bins b)
     const size_t o_a = bl.add(t.a), o_binc = bl.add(binc), o_bini = bl.add(bini);
     const size_t o_cnt = bl.add(cnt), o_bidx = bl.add(bidx), o_bcoef = bl.add(bcoef);
     const size_t o_bI = bl.add(buildItems), o_eI = bl.add(evalItems);
-    const size_t o_dt = bl.add(dtab), o_ex = bl.add(exptab), o_bg = bl.add(bandGrp);
+    const size_t o_dt = bl.add(dtab), o_ex = bl.add(exptab), o_sc = bl.add(sched);
 
     void *blob = nullptr;
     e = cudaMalloc(&blob, bl.bytes.size());
@@ -240,7 +295,7 @@ int upload_tables(cudisc_bins b)
     d.band_idx = (const uint32_t *)(base + o_bidx); d.band_coef = (const double *)(base + o_bcoef);
     d.buildItems = (const uint32_t *)(base + o_bI); d.evalItems = (const uint32_t *)(base + o_eI);
     d.dtab = (const double2 *)(base + o_dt); d.exptab = (const double *)(base + o_ex);
-    d.band_grp = (const int *)(base + o_bg);
+    d.sched = (const int *)(base + o_sc);
     b->dt = d;
     b->dev_blob = blob;
     b->device = dev;
@@ -392,7 +447,7 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
     g->num_sms = sms; g->smem_optin = optin;
 
     const DevTables &d = b->dt;
-    const size_t vec_bytes = smem_vec_doubles(d.Np, d.nchRow, d.nRng, d.nBuildItems + d.nEvalItems) * sizeof(double);
+    const size_t vec_bytes = smem_vec_doubles(d.Np, d.partRowSlots, d.partColSlots, d.nBuildItems + d.nEvalItems) * sizeof(double);
     if (vec_bytes + 16 * 64 > (size_t)optin) {
         delete g;
         return fail(CUDISC_ERR_UNSUPPORTED, "n_bins %d needs %zu B of shared memory", d.N, vec_bytes);

@@ -105,35 +105,44 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         nk = y * s.BINC[BC_RM * Np + k];
         s.NN[k] = nk;
         s.YY[k] = make_double2(y, y * s.BINC[BC_M * Np + k]);
+        s.BANDV[2 * Np + k] = 0.0;                 // second band slot: only split groups write it
+        s.BANDV[2 * Np + N + k] = 0.0;
     }
     if (tid == 0) s.CTR[1] = 0;
     __syncthreads();
     PROF_ADD(2, tp0);
     PROF_T(tpA);
 
-    // ---- phase A: band gather from tensor memory (warp g <-> target group g), then row sums,
-    //      column sums (and, without tensor-memory tables, band gathers) pulled by warps
-    if (tb.bandTmem && 32 * warp < 2 * N) {
-        const int t = 32 * warp + lane;
-        const int Lg = s.CTR[4 + warp], Lp = tb.bandLp;
-        const uint32_t tc = tmem_warp_addr(tbase, warp, 0), ti = tc + 2 * Lp;
-        const double *kd = reinterpret_cast<const double *>(ks.sm);
-        double acc = 0.0;
-        for (int e0 = 0; e0 < Lg; e0 += 8) {
-            uint32_t cf[16], ixs[8];
-            tmem_ld16(tc + 2 * e0, cf);
-            tmem_ld8(ti + e0, ixs);
-            tmem_wait_ld();
+    // ---- phase A: band gathers from tensor memory (tasks fixed per warp: a warp only reaches the
+    //      tensor-memory lanes of its quarter), then row sums, column sums (and, without
+    //      tensor-memory tables, band gathers) pulled by warps
+    if (tb.bandTmem) {
+#pragma unroll 1
+        for (int q = 0; q < 2; ++q) {
+            const int task = s.SCHED[SC_BTASK + 2 * warp + q];
+            if (task >= 0) break;                                  // valid bit = sign bit
+            const int g = (task >> 16) & 0xff, e0b = (task >> 8) & 0xff, e1b = task & 0xff;
+            const int t = 32 * g + lane, Lp = tb.bandLp;
+            const uint32_t tc = tmem_warp_addr(tbase, g, 0), ti = tc + 2 * Lp;
+            const double *kd = reinterpret_cast<const double *>(ks.sm);
+            double acc0 = 0.0, acc1 = 0.0;
+            for (int e0 = e0b; e0 < e1b; e0 += 8) {
+                uint32_t cf[16], ixs[8];
+                tmem_ld16(tc + 2 * e0, cf);
+                tmem_ld8(ti + e0, ixs);
+                tmem_wait_ld();
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const int i = ixs[u] & 0xff, j = (ixs[u] >> 8) & 0xff;
-                const int p2 = 2 * (tri(i) + j) + (int)((ixs[u] >> 16) & 1);
-                const double kv = SLAB ? ((ixs[u] >> 16) & 1 ? ks.ld(p2 >> 1).y : ks.ld(p2 >> 1).x) : kd[p2];
-                const double c = __hiloint2double((int)cf[2 * u + 1], (int)cf[2 * u]);
-                acc = fma(c * s.NN[i], s.NN[j] * kv, acc);
+                for (int u = 0; u < 8; ++u) {
+                    const int i = ixs[u] & 0xff, j = (ixs[u] >> 8) & 0xff;
+                    const int p2 = 2 * (tri(i) + j) + (int)((ixs[u] >> 16) & 1);
+                    const double kv = SLAB ? ((ixs[u] >> 16) & 1 ? ks.ld(p2 >> 1).y : ks.ld(p2 >> 1).x) : kd[p2];
+                    const double c = __hiloint2double((int)cf[2 * u + 1], (int)cf[2 * u]);
+                    if (u & 1) acc1 = fma(c * s.NN[i], s.NN[j] * kv, acc1);
+                    else acc0 = fma(c * s.NN[i], s.NN[j] * kv, acc0);
+                }
             }
+            if (t < 2 * N) s.BANDV[((task >> 30) & 1) * 2 * Np + t] = acc0 + acc1;
         }
-        if (t < 2 * N) s.BANDV[t] = acc;
     }
     for (;;) {
         const int it = next_item(&s.CTR[1], lane);
@@ -146,64 +155,69 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
             const int i = 32 * ix + lane;
             const int jb = kRowChunk * iy;
             int je = 0;
-            if (i < N) je = min(jb + kRowChunk, s.BINI[i].x & 0xffff);
+            if (i < N) je = min(jb + kRowChunk, s.BINI[i].x & 0x1ff);
             const int jmax = iw;                             // max of je over the block (host)
             const int base = tri(i);
-            double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0;
-#pragma unroll 4
-            for (int j = jb; j < jmax; ++j) {
+            double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0, b1 = 0.0, b2 = 0.0, g1 = 0.0, g2 = 0.0;
+#pragma unroll 2
+            for (int j = jb; j < jmax; j += 2) {
                 if (j < je) {
                     const double2 k2 = ks.ld(base + j);
                     const double2 yy = s.YY[j];
                     a1 = fma(k2.x, yy.x, a1); a2 = fma(k2.x, yy.y, a2);
                     f1 = fma(k2.y, yy.x, f1); f2 = fma(k2.y, yy.y, f2);
                 }
+                if (j + 1 < je) {
+                    const double2 k2 = ks.ld(base + j + 1);
+                    const double2 yy = s.YY[j + 1];
+                    b1 = fma(k2.x, yy.x, b1); b2 = fma(k2.x, yy.y, b2);
+                    g1 = fma(k2.y, yy.x, g1); g2 = fma(k2.y, yy.y, g2);
+                }
             }
-            if (i < N) {
-                double2 *pp = reinterpret_cast<double2 *>(s.PARTR + ((size_t)iy * Np + i) * 4);
-                pp[0] = make_double2(a1, a2);
-                pp[1] = make_double2(f1, f2);
+            const int first = s.SCHED[SC_ROWFIRST + iy];
+            if (i < N && i >= first) {
+                double2 *pp = reinterpret_cast<double2 *>(s.PARTR) + 2 * (s.SCHED[SC_ROWOFF + iy] + i - first);
+                pp[0] = make_double2(a1 + b1, a2 + b2);
+                pp[1] = make_double2(f1 + g1, f2 + g2);
             }
         } else if (kind == IT_COL) {
             // lane <-> impactor column j of block ix, target rows i in [iz, iw) of range iy
             const int j = 32 * ix + lane;
-            if (j < N) {
-                const int iSj = s.BINI[j].x >> 16;
-                double gc = 0.0, h = 0.0;
-#pragma unroll 4
-                for (int i = max(iz, j); i < iw; ++i) {
+            if (j < min(N, iw)) {
+                const int iSj = (s.BINI[j].x >> 9) & 0x1ff;
+                double gc = 0.0, h = 0.0, gc2 = 0.0, h2 = 0.0;
+                int i = max(iz, j);
+                if ((iw - i) & 1) {
                     const double2 k2 = ks.ld(tri(i) + j);
                     const double ni = s.NN[i];
                     gc = fma(k2.x, ni, gc);
                     if (i >= iSj) h = fma(k2.y, ni, h);
+                    ++i;
                 }
-                reinterpret_cast<double2 *>(s.PARTC)[(size_t)iy * Np + j] = make_double2(gc, h);
+#pragma unroll 2
+                for (; i < iw; i += 2) {
+                    const double2 k2 = ks.ld(tri(i) + j), k3 = ks.ld(tri(i + 1) + j);
+                    const double ni = s.NN[i], ni1 = s.NN[i + 1];
+                    gc = fma(k2.x, ni, gc);
+                    if (i >= iSj) h = fma(k2.y, ni, h);
+                    gc2 = fma(k3.x, ni1, gc2);
+                    if (i + 1 >= iSj) h2 = fma(k3.y, ni1, h2);
+                }
+                reinterpret_cast<double2 *>(s.PARTC)[s.SCHED[SC_COLOFF + iy] + j] = make_double2(gc + gc2, h + h2);
             }
         } else {
-            // band gather: lane <-> target t of group ix (t < N: bins, t >= N: S bins)
+            // band gather from global tables (fallback): lane <-> target t of group ix
             const int t = 32 * ix + lane;
             const int cnt = (t < 2 * N) ? __ldg(tb.band_cnt + t) : 0;
-            const int cmax = iw;
-            const uint32_t *pi = tb.band_idx + t;
-            const double *pcf = tb.band_coef + t;
             double acc = 0.0;
-            for (int e0 = 0; e0 < cmax; e0 += 8) {
-                uint32_t ixs[8];
-                double cfs[8];
-#pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const bool on = e0 + u < cnt;
-                    ixs[u] = on ? __ldcg(pi + (size_t)(e0 + u) * tb.bandW) : 0u;
-                    cfs[u] = on ? __ldcg(pcf + (size_t)(e0 + u) * tb.bandW) : 0.0;
-                }
-#pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    if (e0 + u < cnt) {
-                        const int i = ixs[u] & 0xff, j = (ixs[u] >> 8) & 0xff;
-                        const double2 k2 = ks.ld(tri(i) + j);
-                        const double kv = (ixs[u] >> 16) & 1 ? k2.y : k2.x;
-                        acc = fma(cfs[u] * s.NN[i], s.NN[j] * kv, acc);
-                    }
+            for (int e = 0; e < iw; ++e) {
+                if (e < cnt) {
+                    const uint32_t ixe = __ldcg(tb.band_idx + (size_t)e * tb.bandW + t);
+                    const double cf = __ldcg(tb.band_coef + (size_t)e * tb.bandW + t);
+                    const int i = ixe & 0xff, j = (ixe >> 8) & 0xff;
+                    const double2 k2 = ks.ld(tri(i) + j);
+                    const double kv = (ixe >> 16) & 1 ? k2.y : k2.x;
+                    acc = fma(cf * s.NN[i], s.NN[j] * kv, acc);
                 }
             }
             if (t < 2 * N) s.BANDV[t] = acc;
@@ -218,10 +232,11 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, G = 0.0, sv = 0.0;
     if (live) {
         const int2 bi = s.BINI[k];
-        const int nch = ((bi.x & 0xffff) + kRowChunk - 1) / kRowChunk;
+        const int nch = ((bi.x & 0x1ff) + kRowChunk - 1) / kRowChunk;
         double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0;
         for (int c = 0; c < nch; ++c) {
-            const double2 *pp = reinterpret_cast<const double2 *>(s.PARTR + ((size_t)c * Np + k) * 4);
+            const double2 *pp = reinterpret_cast<const double2 *>(s.PARTR)
+                                + 2 * (s.SCHED[SC_ROWOFF + c] + k - s.SCHED[SC_ROWFIRST + c]);
             const double2 u = pp[0], v = pp[1];
             a1 += u.x; a2 += u.y; f1 += v.x; f2 += v.y;
         }
@@ -230,22 +245,22 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         dm1 = nk * (bc[BC_G1 * Np] * f1 - cF2 * f2);
         d0 = nk * ((bc[BC_A1 * Np] * a1 + cA2 * a2) + (bc[BC_F1 * Np] * f1 + cF2 * f2));
         dp1 = nk * (bc[BC_B1 * Np] * a1 - cA2 * a2);
-        // column sums of bin j over the row ranges that reach rows >= j (fixed order)
-        auto colsum = [&](int j, double &gj, double &hj) {
+        // column sums of bin j over the row ranges that hold rows >= j (fixed order)
+        auto colsum = [&](int j, int rfirst, double &gj, double &hj) {
             gj = 0.0; hj = 0.0;
-            for (int r = (j & ~31) / tb.rngLen; r < tb.nRng; ++r) {
-                const double2 u = reinterpret_cast<const double2 *>(s.PARTC)[(size_t)r * Np + j];
+            for (int r = rfirst; r < tb.nRng; ++r) {
+                const double2 u = reinterpret_cast<const double2 *>(s.PARTC)[s.SCHED[SC_COLOFF + r] + j];
                 gj += u.x; hj += u.y;
             }
         };
         double gc, h;
-        colsum(k, gc, h);
+        colsum(k, bi.x >> 18, gc, h);
         G = gc + h;
         // fragment source of l-bin k, scaled by 1/B_k
-        double sl = s.BANDV[N + k];
+        double sl = s.BANDV[N + k] + s.BANDV[2 * Np + N + k];
         for (int j = bi.y & 0xffff; j < (bi.y >> 16); ++j) {
             double gj, hj = h;
-            if (j != k) colsum(j, gj, hj);
+            if (j != k) colsum(j, s.BINI[j].x >> 18, gj, hj);
             sl = fma(tb.sS * s.YY[j].x, hj, sl);
         }
         sv = sl * bc[BC_FIB * Np];
@@ -273,7 +288,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         d = d0;
         if (k > 0) d += prev;
         if (k < N - 1) d += next;
-        d += s.BANDV[k];
+        d += s.BANDV[k] + s.BANDV[2 * Np + k];
         d = fma(-y, G, d);
         d = fma(s.BINC[BC_FA * Np + k], suf, d);
     }
@@ -292,7 +307,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
     ks.sm = reinterpret_cast<double2 *>(smem_raw);
     ks.Psm = sa.Psm;
     ks.gl = reinterpret_cast<double2 *>(sa.kslab) + (size_t)blockIdx.x * (size_t)(P - sa.Psm);
-    const Smem s = carve(smem_raw + 2 * (size_t)sa.Psm, tb.Np, tb.nchRow, tb.nRng, tb.nBuildItems,
+    const Smem s = carve(smem_raw + 2 * (size_t)sa.Psm, tb.Np, tb.partRowSlots, tb.nBuildItems,
                          tb.nEvalItems);
     PairConst pc;
     const bool has_vphi = gs.vphi != nullptr;
@@ -306,7 +321,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
     for (int q = tid; q < N; q += NT) s.BINI[q] = tb.bini[q];
     for (int q = tid; q < tb.nBuildItems; q += NT) s.ITB[q] = tb.buildItems[q];
     for (int q = tid; q < tb.nEvalItems; q += NT) s.ITE[q] = tb.evalItems[q];
-    if (tid < 16) s.CTR[4 + tid] = tb.band_grp[tid];
+    if (tid < kSched) s.SCHED[tid] = tb.sched[tid];
     // band tables -> tensor memory (grid-only constants, once per CTA)
     uint32_t tbase = 0;
     const bool use_tmem = MODE != MODE_KERNEL && tb.bandTmem;
