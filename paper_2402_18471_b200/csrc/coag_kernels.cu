@@ -36,10 +36,10 @@ __device__ __forceinline__ void build_items(const DevTables &tb, const Smem &s, 
             const RoleJ B = load_role_j<VPHI>(s, valid ? j : N - 1);
             for (int i = ia; i < ib; i += 2) {
                 const int i2 = min(i + 1, ib - 1);
-                const RoleI A1 = load_role_i<VPHI>(s, i);
-                const RoleI A2 = load_role_i<VPHI>(s, i2);
-                const double2 k1 = pair_kernel<VPHI, LOG>(A1, B, i - j, pc, s);
-                const double2 k2 = pair_kernel<VPHI, LOG>(A2, B, i2 - j, pc, s);
+                const RoleI A1 = load_role_i<VPHI, false>(s, i);
+                const RoleI A2 = load_role_i<VPHI, false>(s, i2);
+                const double2 k1 = pair_kernel<VPHI, LOG, false>(A1, B, i - j, pc, s);
+                const double2 k2 = pair_kernel<VPHI, LOG, false>(A2, B, i2 - j, pc, s);
                 if (valid) {
                     const int p1 = tri(i) + j, p2 = tri(i2) + j;
                     if (MODE == MODE_KERNEL) {
@@ -57,9 +57,9 @@ __device__ __forceinline__ void build_items(const DevTables &tb, const Smem &s, 
                 r += (tri(r + 1) <= t) ? 1 : 0;
                 r -= (tri(r) > t) ? 1 : 0;
                 const int i = 32 * c + r, j = 32 * c + (t - tri(r));
-                const RoleI A = load_role_i<VPHI>(s, i);
+                const RoleI A = load_role_i<VPHI, true>(s, i);
                 const RoleJ B = load_role_j<VPHI>(s, j);
-                double2 k2 = pair_kernel<VPHI, LOG>(A, B, i - j, pc, s);
+                double2 k2 = pair_kernel<VPHI, LOG, true>(A, B, i - j, pc, s);
                 const int p = tri(i) + j;
                 if (MODE == MODE_KERNEL) {
                     kout[p] = k2.x; kout[P + p] = k2.y;
