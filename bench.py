@@ -40,7 +40,7 @@ import numpy as np  # noqa: E402
 
 # Algorithmic FP64 instruction counts of the minimal pair formulas (an FMA,
 # add, mul or max each count 1; per-bin hoistable terms excluded).
-I_BUILD = 59      # per pair, once per step: Eqs. 56-62
+I_BUILD = 41      # per pair, once per step: Eqs. 56-62 on a log grid (FP64-pipe instructions of pair_kernel)
 I_EVAL = 6        # per pair per rate evaluation: 4 row-sum + 2 column-sum FMAs
 EVALS_PER_STEP = 3
 FP64_LANES_PER_SM = 64
@@ -305,7 +305,7 @@ def run_ours(args):
                     "api": "cudisc_coag_step_host (pinned host buffers)"},
             "gpu_launches": int(launches),
             "roofline": {
-                "bound": "alu", "kernel": "cudisc::coag_cells_kernel<512, MODE_STEP>",
+                "bound": "alu", "kernel": "cudisc::coag_cells_kernel<512, MODE_STEP, false>",
                 "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops, "traffic": None,
                 "how": f"algorithmic FP64 instructions per launch = C*P*({I_BUILD} + {EVALS_PER_STEP}*{I_EVAL}) "
@@ -316,6 +316,9 @@ def run_ours(args):
                 "frac_of_measured_dfma": achieved_tflops / (2.0 * dfma_per_s / 1e12),
                 "hbm_copy_measured_gbs": copy_bps / 1e9,
                 "hbm_algorithmic_gbs": (6.0 * C * N * 8 + 5.0 * C * 8) / kernel_s / 1e9,
+                "note": "the FP64 pipe is the roofline BASELINE.json names; ncu (profiles/) shows the kernel is "
+                        "limited by the shared-memory data pipe (K store read twice per rate evaluation), "
+                        "see DESIGN.md 'Roofline'",
             },
         }
         if world == 1 and not args.no_cpu_baseline:

@@ -116,6 +116,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     // ---- phase A: band gathers from tensor memory (tasks fixed per warp: a warp only reaches the
     //      tensor-memory lanes of its quarter), then row sums, column sums (and, without
     //      tensor-memory tables, band gathers) pulled by warps
+#ifndef CUDISC_NOBAND
     if (tb.bandTmem) {
 #pragma unroll 1
         for (int q = 0; q < 2; ++q) {
@@ -144,6 +145,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
             if (t < 2 * N) s.BANDV[((task >> 30) & 1) * 2 * Np + t] = acc0 + acc1;
         }
     }
+#endif
     for (;;) {
         const int it = next_item(&s.CTR[1], lane);
         if (it >= tb.nEvalItems) break;
@@ -159,7 +161,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
             const int jmax = iw;                             // max of je over the block (host)
             const int base = tri(i);
             double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0, b1 = 0.0, b2 = 0.0, g1 = 0.0, g2 = 0.0;
-#pragma unroll 2
+#pragma unroll 4
             for (int j = jb; j < jmax; j += 2) {
                 if (j < je) {
                     const double2 k2 = ks.ld(base + j);
@@ -194,7 +196,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
                     if (i >= iSj) h = fma(k2.y, ni, h);
                     ++i;
                 }
-#pragma unroll 2
+#pragma unroll 4
                 for (; i < iw; i += 2) {
                     const double2 k2 = ks.ld(tri(i) + j), k3 = ks.ld(tri(i + 1) + j);
                     const double ni = s.NN[i], ni1 = s.NN[i + 1];
