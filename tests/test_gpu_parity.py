@@ -146,3 +146,102 @@ def test_bit_reproducible_run_to_run():
         err = g.step(rho, dt_of(4))
         outs.append((rho.clone(), err.clone()))
     assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+
+
+# ------------------------------------------------------------------------------------------ other grids, edge sizes
+def _manual_inputs(N, C, seed, a_min=1e-5, a_max=10.0, T0=60.0):
+    """Seeded inputs for sizes the five configs do not cover (recipe: log-uniform gas state, normal
+    velocities, lognormal densities; no method arithmetic)."""
+    rng = np.random.default_rng(seed)
+    T = T0 * np.exp(rng.uniform(-0.5, 0.5, C))
+    rho_g = 10.0 ** rng.uniform(-15.0, -10.5, C)
+    Om = 10.0 ** rng.uniform(-9.5, -8.0, C)
+    alpha = np.full(C, 1e-3)
+    vR = rng.normal(scale=30.0, size=(C, N)) * np.linspace(0.01, 1.0, N)
+    vZ = rng.normal(scale=30.0, size=(C, N)) * np.linspace(0.01, 1.0, N)
+    rho = 1e-14 * np.exp(rng.normal(scale=2.0, size=(C, N)))
+    return dict(T=T, rho_gas=rho_g, Omega=Om, alpha=alpha, v_R=vR, v_Z=vZ, rho=rho, a_min=a_min, a_max=a_max)
+
+
+def _run_manual(N, C, seed, n_r=None, n_z=None, m_centres=None, m_edges=None, steps=1, dt=1.0e5):
+    import torch
+    inp = _manual_inputs(N, C, seed)
+    po = orc.Params(v_frag=100.0)
+    pc = cd.Params(v_frag=100.0, alpha=1e-3)
+    rho_m = 1.67
+    bins = cd.Bins(N, inp["a_min"], inp["a_max"], rho_m, pc, m_centres=m_centres, m_edges=m_edges)
+    grid = cd.Grid(n_r or C, n_z or 1, bins)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    gas = dict(T=t(inp["T"]), rho_gas=t(inp["rho_gas"]), Omega=t(inp["Omega"]), alpha=t(inp["alpha"]),
+               v_R=t(inp["v_R"]), v_Z=t(inp["v_Z"]))
+    grid.bind_gas(**gas)
+    # oracle, cell by cell, on the library's own grid description (masses and radii are inputs)
+    q = bins.query()
+    g = orc.MassGrid(N, np.zeros(N + 1), q["m_edges"], q["a_centres"], q["m_centres"], rho_m, 0.0, 0.0)
+    K = torch.empty((C, 2, bins.n_pairs), dtype=torch.float64, device="cuda")
+    cd.cudisc_coag_kernel(grid, bins, gas, pc, K)
+    drho = torch.empty((C, N), dtype=torch.float64, device="cuda")
+    rho = t(inp["rho"])
+    cd.cudisc_coag_rates_otf(grid, bins, rho, drho)
+    err = torch.empty(C, dtype=torch.float64, device="cuda")
+    y = rho.clone()
+    for _ in range(steps):
+        cd.cudisc_coag_step(grid, bins, y, dt, err)
+    torch.cuda.synchronize()
+    K = K.cpu().numpy(); drho = drho.cpu().numpy(); y = y.cpu().numpy(); err = err.cpu().numpy()
+    iu = np.tril_indices(N)
+    for c in range(C):
+        Kc, pf, _, _ = orc.cell_kernel(g, inp["T"][c], inp["rho_gas"][c], inp["Omega"][c], inp["alpha"][c],
+                                       inp["v_R"][c], inp["v_Z"][c], po)
+        Kt = Kc[iu]
+        assert np.all(np.abs(K[c, 1] - (Kc * pf)[iu]) <= TOL_K * Kt), f"cell {c} Kf"
+        assert np.all(np.abs(K[c, 0] - (Kc * (1.0 - pf))[iu]) <= TOL_K * Kt), f"cell {c} Kc"
+        d, _, _, _ = orc.rates_flux(g, Kc, pf, inp["rho"][c])
+        _, gain, loss, _ = orc.rates_flux(g, Kc, 0.5 * np.ones_like(pf), inp["rho"][c])   # split-free scale
+        assert_rates_close(drho[c:c + 1], d[None], 2.0 * gain[None], 2.0 * loss[None], what=f"cell {c} rates")
+        yr, k1, E = inp["rho"][c].copy(), None, 0.0
+        for _ in range(steps):
+            yr, k1, E = orc.bs32_step(g, Kc, pf, yr, dt, k1=k1)
+        assert_rho_close(y[c:c + 1], yr[None], TOL_RHO_1 * steps, f"cell {c} step")
+        assert abs(err[c] - E) <= 1e-6 * abs(E) + 1e-12
+        m0 = inp["rho"][c].sum()
+        assert abs(y[c].sum() - m0) <= steps * TOL_MASS * m0
+
+
+@pytest.mark.parametrize("N,C", [(2, 3), (33, 5), (64, 200), (256, 4)])
+def test_edge_sizes_log_grid(N, C):
+    """Minimum bin count, a ragged 32-multiple, more cells than SMs, and the maximum bin count
+    (band tables too long for tensor memory -> global-table gather; K store partly in the L2 slab)."""
+    _run_manual(N, C, seed=100 + N, steps=2)
+
+
+def test_general_mass_grid_matches_oracle():
+    """cudisc_bins_create_general: a non-log grid takes the table-free sigma / Stokes-ratio path."""
+    N = 48
+    ge = orc.mass_grid(N, 1e-5, 10.0, 1.67)
+    wob = 1.0 + 0.04 * np.sin(1.7 * np.arange(N + 1))
+    m_e = ge.m_e * wob
+    m_c = np.sqrt(m_e[:-1] * m_e[1:]) * (1.0 + 0.01 * np.cos(2.3 * np.arange(N)))
+    assert np.all(np.diff(m_e) > 0) and np.all(m_e[:-1] < m_c) and np.all(m_c < m_e[1:])
+    _run_manual(N, 6, seed=7, m_centres=m_c, m_edges=m_e, steps=2)
+
+
+def test_full_grid_launch_configuration_sampled_against_oracle():
+    """BASELINE.json config 4 at full size (32000 cells x 150 bins), the launch bench.py times:
+    one step on the whole grid, checked on sampled cells the oracle computes one by one."""
+    cfg = synth_disc.CONFIGS[4]
+    d = synth_disc.make_disc(4)
+    po, pc = params_pair(cfg)
+    g = GpuDisc(d, pc, n_r=cfg.n_r, n_z=cfg.n_z)
+    dt = dt_of(4)
+    rho = g.rho.clone()
+    err = g.step(rho, dt).cpu().numpy()
+    rho = rho.cpu().numpy()
+    cells = synth_disc.sample_cells(cfg, 40, seed=11)
+    ds = d.subset(cells)
+    rho_ref, _, err_ref = orc.step_cells(*oracle_args(ds), po, ds.rho_dust, dt)
+    assert_rho_close(rho[cells], rho_ref, TOL_RHO_1, "cfg4 full grid, sampled cells")
+    np.testing.assert_allclose(err[cells], err_ref, rtol=1e-6, atol=1e-12)
+    m0 = d.rho_dust.sum(axis=1)
+    assert np.max(np.abs(rho.sum(axis=1) - m0) / m0) <= TOL_MASS
+    assert np.all(np.isfinite(rho)) and np.all(np.isfinite(err))
