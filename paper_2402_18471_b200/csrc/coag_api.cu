@@ -238,6 +238,8 @@ int upload_tables(cudisc_bins b)
     {
         constexpr int nWarps = kThreads / 32;
         int load[nWarps] = {0}, ntask[nWarps] = {0};
+        // the bin-owning warps also compute the next cell's per-bin values during the last evaluation
+        for (int w = 0; w < nWarps; ++w) load[w] = (32 * w < N) ? 12 : 0;
         for (int tg = 0; tg < nGroups; ++tg) {
             int cmax = 0;
             for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
@@ -469,8 +471,8 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
         return cuda_fail(e, "cudaMalloc(grid)");
     }
 #ifdef CUDISC_PROF
-    cudaMalloc((void **)&g->prof, (size_t)g->grid_ctas * 16 * sizeof(long long));
-    cudaMemset(g->prof, 0, (size_t)g->grid_ctas * 16 * sizeof(long long));
+    cudaMalloc((void **)&g->prof, (size_t)g->grid_ctas * 48 * sizeof(long long));
+    cudaMemset(g->prof, 0, (size_t)g->grid_ctas * 48 * sizeof(long long));
 #endif
     *out = g;
     return CUDISC_OK;
@@ -482,8 +484,8 @@ int cudisc_debug_prof(cudisc_grid g, long long *out_host, int n_ctas)
 {
     cudaDeviceSynchronize();
     n_ctas = std::min(n_ctas, g->grid_ctas);
-    cudaMemcpy(out_host, g->prof, (size_t)n_ctas * 16 * sizeof(long long), cudaMemcpyDeviceToHost);
-    cudaMemset(g->prof, 0, (size_t)g->grid_ctas * 16 * sizeof(long long));
+    cudaMemcpy(out_host, g->prof, (size_t)n_ctas * 48 * sizeof(long long), cudaMemcpyDeviceToHost);
+    cudaMemset(g->prof, 0, (size_t)g->grid_ctas * 48 * sizeof(long long));
     return n_ctas;
 }
 #endif

@@ -91,7 +91,9 @@ __device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, c
 // Three block barriers; every partial sum has its own slot and every combination a fixed order.
 template <int NT, bool SLAB>
 __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
-                                             double y, int tid, uint32_t tbase, long long *sa_prof)
+                                             double y, int tid, uint32_t tbase, long long *sa_prof,
+                                             bool pre, const CellGas &nx, double mu, double sigma_mol,
+                                             RoleVals &rv)
 {
     PROF_T(tp0);
     const int N = tb.N, Np = tb.Np;
@@ -112,6 +114,10 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     __syncthreads();
     PROF_ADD(2, tp0);
     PROF_T(tpA);
+
+    // per-bin values of the NEXT cell (inputs were fetched an evaluation ago): the bin-owning warps
+    // compute them here, in registers, while the other warps start on the items
+    if (pre && 32 * warp < N) rv = prologue_compute(tb, nx, mu, sigma_mol, s, k);
 
     // ---- phase A: band gathers from tensor memory (tasks fixed per warp: a warp only reaches the
     //      tensor-memory lanes of its quarter), then row sums, column sums (and, without
@@ -226,6 +232,9 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         }
     }
     PROF_ADD(3, tpA);
+#ifdef CUDISC_PROF
+    if (lane == 0) sa_prof[16 + warp] += clock64() - tpA;
+#endif
     __syncthreads();
     PROF_ADD(4, tpA);
     PROF_T(tpB);
@@ -368,7 +377,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
     __syncthreads();
     if (use_tmem) tmem_fence_after();
 
-    long long *sa_prof = sa.prof ? sa.prof + 16 * (size_t)blockIdx.x : nullptr;
+    long long *sa_prof = sa.prof ? sa.prof + 48 * (size_t)blockIdx.x : nullptr;
     (void)sa_prof;
     const int k = tid;
     const bool live = k < N;
@@ -388,6 +397,9 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
         }
     };
     fetch(blockIdx.x);
+    RoleVals rv;
+    rv.Vg2 = 0.0;
+    bool rv_valid = false;       // rv holds the next cell's values (computed during the last evaluation)
 
     for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
         PROF_T(tc0);
@@ -404,9 +416,12 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
                 }
             }
         } else {
-            pc.Vg2 = cell_prologue(tb, nx, gs.mu, gs.sigma_mol, nvR, nvZ, nvP, has_vphi, s, k);
-            if (tid == 0) s.CTR[0] = 0;
+            if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, s, k);
+            prologue_store(tb, rv, nvR, nvZ, nvP, has_vphi, s, k);
+            // V_g^2 through shared memory: only the bin-owning warps hold the pre-computed values
+            if (tid == 0) { s.CTR[0] = 0; reinterpret_cast<double *>(s.CTR)[1] = rv.Vg2; }
             __syncthreads();
+            pc.Vg2 = reinterpret_cast<const double *>(s.CTR)[1];
             PROF_ADD(0, tc0);
         }
         // state (thread <-> bin): in flight during the build
@@ -425,7 +440,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
 
         if (MODE == MODE_RATES || MODE == MODE_OTF) {
             fetch(cell + gridDim.x);
-            const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, tbase, sa_prof);
+            const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, tbase, sa_prof, false, nx, gs.mu, gs.sigma_mol, rv);
             if (live) sa.out[row + k] = d;
             __syncthreads();
             continue;
@@ -439,12 +454,15 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
             double ys = y0;
             if (st == 1) ys = y0 + 0.5 * h * k1;
             if (st == 2) ys = y0 + 0.75 * h * k2;
+            if (st == 2) fetch(cell + gridDim.x);
             if (st == 3) {
                 yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
                 ys = yn;
-                fetch(cell + gridDim.x);
             }
-            const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, tbase, sa_prof);
+            const bool pre = st == 3 && cell + (int)gridDim.x < sa.C;
+            const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, tbase, sa_prof, pre, nx, gs.mu,
+                                                  gs.sigma_mol, rv);
+            if (st == 3) rv_valid = pre;
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;
             if (st == 2) k3 = d;
