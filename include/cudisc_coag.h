@@ -172,6 +172,38 @@ int cudisc_coag_step_host(cudisc_grid g, cudisc_bins b, double *rho_host, double
                           double *err_host, cudisc_stream stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Adaptive sub-cycling (reading R10)
+ * ------------------------------------------------------------------------------------------- */
+
+typedef struct {
+    double t_done;        /* time covered, s (== t_span unless max_steps ran out)                  */
+    double dt_last;       /* size of the last accepted step (possibly truncated to land on t_span) */
+    double dt_next;       /* the controller's suggestion for the next step: hand it back as dt_try
+                             of the next call ("the final sub-timestep")             */
+    double err_last;      /* max_c E_c of the last accepted step                                   */
+    int n_accepted, n_rejected;
+} cudisc_integrate_info;
+
+/* Step-size controller of the embedded pair (R10, textbook): a step of size h with error norm
+ * E = max_c E_c is accepted iff E <= 1; the next trial size is h * clamp(0.9 E^(-1/3), 0.2, 5)
+ * (factor 5 for E == 0).  Pure host function, no device needed. */
+double cudisc_controller_next_dt(double E, double h);
+
+/* Integrates every cell over t_span seconds with adaptive BS3(2) sub-steps of ONE global size
+ * (coagulation sub-cycles inside the global step with the gas state frozen).
+ * Each trial step is one cudisc_coag_step launch into trial buffers owned by g, a max-reduction of
+ * the per-cell error norms on the device and an 8-byte read-back; rejected steps leave the state
+ * untouched.  The last step is cut to land on t_span.
+ * rho_dust: DEVICE [C x N] in/out.  dt_try: first trial size, s (> 0).  max_steps: bound on accepted
+ * + rejected steps.  dt_log: HOST [max_steps] or NULL; receives the size of every trial step in
+ * order, negated when the step was rejected.  info: HOST, may be NULL.
+ * SYNCHRONISES with `stream` (once per trial step).  A non-finite error norm stops the
+ * integration with CUDISC_ERR_INVALID (rho_dust then holds the last accepted state). */
+int cudisc_coag_integrate(cudisc_grid g, cudisc_bins b, double *rho_dust, double t_span, double dt_try,
+                          int max_steps, double *dt_log, cudisc_integrate_info *info,
+                          cudisc_stream stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Roofline denominators measured in the same process (north_star: "peaks measured by a
  * microbenchmark in the same run").  Both synchronise the device.
  * ------------------------------------------------------------------------------------------- */

@@ -282,3 +282,48 @@ def pack_planes(K: np.ndarray, pf: np.ndarray) -> np.ndarray:
     N = K.shape[0]
     il = np.tril_indices(N)
     return np.ascontiguousarray(np.stack([(K * (1.0 - pf))[il], (K * pf)[il]]))
+
+
+# ------------------------------------------------------------------------------------------ adaptive sub-cycling
+def controller_next_dt(E: float, h: float) -> float:
+    """Step-size controller of the embedded pair (R10; PAPER.md:478 names the method and the
+    tolerances only): next trial size h * clamp(0.9 E^(-1/3), 0.2, 5), factor 5 for E = 0.  A step is
+    accepted iff E <= 1.  Pins: E = 0.729 keeps h (0.9 / 0.9); E = 1 gives 0.9 h; clamps at 0.2 and 5."""
+    f = 5.0 if E <= 0.0 else 0.9 * E ** (-1.0 / 3.0)
+    return h * min(5.0, max(0.2, f))
+
+
+def integrate(step, rho, t_span: float, dt_try: float, max_steps: int = 100000):
+    """Adaptive sub-cycling over t_span with ONE global step size: `step(rho, dt, k1)` is
+    one BS3(2) step of every cell returning (rho_new, k4, err[C]); the global error norm is max_c err_c;
+    the last step is cut to land on t_span (a cut step does not shrink the next trial size).
+    Returns rho, list of trial step sizes (negative = rejected), dt_next."""
+    t, dt, k1, log = 0.0, float(dt_try), None, []
+    rho = np.array(rho, dtype=np.float64, copy=True)
+    while t < t_span and len(log) < max_steps:
+        left = t_span - t
+        cut = dt >= left
+        h = left if cut else dt
+        rho_new, k4, err = step(rho, h, k1)
+        E = float(np.max(err))
+        if not np.isfinite(E):
+            raise FloatingPointError("non-finite error norm")
+        if E <= 1.0:
+            rho, k1 = rho_new, k4
+            t = t_span if cut else t + h
+            log.append(h)
+            sug = controller_next_dt(E, h)
+            dt = max(sug, dt) if cut else sug
+        else:
+            log.append(-h)
+            dt = controller_next_dt(E, h)
+    return rho, log, dt
+
+
+def replay(step, rho, dts):
+    """Fixed schedule: the accepted steps of a recorded run (parity under adaptivity)."""
+    rho = np.array(rho, dtype=np.float64, copy=True)
+    k1 = None
+    for h in dts:
+        rho, k1, _ = step(rho, float(h), k1)
+    return rho

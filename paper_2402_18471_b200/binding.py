@@ -36,11 +36,17 @@ class cudisc_gas_state(C.Structure):
                 ("v_R", C.c_void_p), ("v_Z", C.c_void_p), ("v_phi", C.c_void_p)]
 
 
+class cudisc_integrate_info(C.Structure):
+    _fields_ = [("t_done", C.c_double), ("dt_last", C.c_double), ("dt_next", C.c_double),
+                ("err_last", C.c_double), ("n_accepted", C.c_int), ("n_rejected", C.c_int)]
+
+
 EXPORTS = [
     "cudisc_bins_create", "cudisc_bins_create_general", "cudisc_bins_destroy", "cudisc_bins_query",
     "cudisc_bins_expand_outcomes", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
     "cudisc_grid_destroy", "cudisc_coag_kernel", "cudisc_coag_rates", "cudisc_coag_rates_otf",
-    "cudisc_coag_step", "cudisc_coag_step_host", "cudisc_microbench_dfma",
+    "cudisc_coag_step", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_controller_next_dt",
+    "cudisc_microbench_dfma",
     "cudisc_microbench_copy", "cudisc_launch_count", "cudisc_last_error", "cudisc_version",
 ]
 
@@ -70,6 +76,10 @@ def lib() -> C.CDLL:
         L.cudisc_coag_rates_otf.argtypes = [vp, vp, vp, vp, vp]
         L.cudisc_coag_step.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.cudisc_coag_step_host.argtypes = [vp, vp, vp, C.c_double, vp, vp]
+        L.cudisc_coag_integrate.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int, dp,
+                                            C.POINTER(cudisc_integrate_info), vp]
+        L.cudisc_controller_next_dt.argtypes = [C.c_double, C.c_double]
+        L.cudisc_controller_next_dt.restype = C.c_double
         L.cudisc_microbench_dfma.argtypes = [C.c_int, dp, dp]
         L.cudisc_microbench_copy.argtypes = [C.c_longlong, dp, dp]
         L.cudisc_launch_count.restype = C.c_longlong
@@ -269,6 +279,25 @@ def cudisc_coag_step_host(grid: Grid, bins: Bins, rho_host, dt: float, err_host,
     Cn, N = grid.n_cells, bins.n_bins
     _check(lib().cudisc_coag_step_host(grid.handle, bins.handle, _host_ptr(rho_host, "rho_host", Cn * N),
                                        float(dt), _host_ptr(err_host, "err_host", Cn), _stream(stream)))
+
+
+def cudisc_controller_next_dt(E: float, h: float) -> float:
+    return float(lib().cudisc_controller_next_dt(float(E), float(h)))
+
+
+def cudisc_coag_integrate(grid: Grid, bins: Bins, rho_dust, t_span: float, dt_try: float, max_steps: int = 10000,
+                          stream=None):
+    """Adaptive BS3(2) sub-cycling over t_span.  Returns (info dict, dt_log): dt_log holds
+    the size of every trial step, negated when rejected."""
+    Cn, N = grid.n_cells, bins.n_bins
+    log = np.zeros(max_steps)
+    info = cudisc_integrate_info()
+    _check(lib().cudisc_coag_integrate(grid.handle, bins.handle, _dev_ptr(rho_dust, "rho_dust", Cn * N),
+                                       float(t_span), float(dt_try), int(max_steps),
+                                       log.ctypes.data_as(C.POINTER(C.c_double)), C.byref(info), _stream(stream)))
+    n = info.n_accepted + info.n_rejected
+    return ({"t_done": info.t_done, "dt_last": info.dt_last, "dt_next": info.dt_next, "err_last": info.err_last,
+             "n_accepted": info.n_accepted, "n_rejected": info.n_rejected}, log[:n].copy())
 
 
 def cudisc_microbench_dfma(n_iter: int = 0):

@@ -64,6 +64,8 @@ struct cudisc_grid_s {
     double *kslab;      // per-CTA overflow of the K store
     double *stage_rho;  // [C x N] staging of cudisc_coag_step_host (lazy)
     double *stage_err;  // [C]
+    double *trial_rho, *trial_k, *trial_err, *d_emax;   // cudisc_coag_integrate (lazy)
+    double *h_emax;     // pinned host scalar
     long long *prof;    // CUDISC_PROF builds only
     int num_sms, smem_optin, grid_ctas, Psm, smem_bytes;
 };
@@ -446,6 +448,7 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
     g->gas_bound = false; g->fsal_valid = false;
     g->k_fsal = nullptr; g->kslab = nullptr;
     g->stage_rho = nullptr; g->stage_err = nullptr; g->prof = nullptr;
+    g->trial_rho = g->trial_k = g->trial_err = g->d_emax = g->h_emax = nullptr;
     g->num_sms = sms; g->smem_optin = optin;
 
     const DevTables &d = b->dt;
@@ -516,6 +519,11 @@ int cudisc_grid_destroy(cudisc_grid g)
     if (g->stage_rho) cudaFree(g->stage_rho);
     if (g->stage_err) cudaFree(g->stage_err);
     if (g->prof) cudaFree(g->prof);
+    if (g->trial_rho) cudaFree(g->trial_rho);
+    if (g->trial_k) cudaFree(g->trial_k);
+    if (g->trial_err) cudaFree(g->trial_err);
+    if (g->d_emax) cudaFree(g->d_emax);
+    if (g->h_emax) cudaFreeHost(g->h_emax);
     g->magic = 0;
     delete g;
     return CUDISC_OK;
@@ -610,6 +618,88 @@ int cudisc_coag_step_host(cudisc_grid g, cudisc_bins b, double *rho_host, double
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return cuda_fail(e, "step_host copies");
     return CUDISC_OK;
+}
+
+double cudisc_controller_next_dt(double E, double h)
+{
+    double f = 5.0;
+    if (E > 0.0) f = 0.9 * std::pow(E, -1.0 / 3.0);
+    f = std::min(5.0, std::max(0.2, f));
+    return h * f;
+}
+
+int cudisc_coag_integrate(cudisc_grid g, cudisc_bins b, double *rho_dust, double t_span, double dt_try,
+                          int max_steps, double *dt_log, cudisc_integrate_info *info, cudisc_stream stream)
+{
+    int rc = check_pair(g, b);
+    if (rc) return rc;
+    if (!g->gas_bound) return fail(CUDISC_ERR_INVALID, "no gas state bound (cudisc_grid_bind_gas)");
+    if (!rho_dust) return fail(CUDISC_ERR_INVALID, "NULL array argument");
+    if (!(t_span > 0.0) || !(dt_try > 0.0) || max_steps < 1)
+        return fail(CUDISC_ERR_INVALID, "need t_span > 0, dt_try > 0, max_steps >= 1");
+    const size_t row_bytes = (size_t)g->C * b->ht.N * sizeof(double);
+    cudaError_t e = cudaSuccess;
+    if (!g->trial_rho) {
+        e = cudaMalloc((void **)&g->trial_rho, row_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g->trial_k, row_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g->trial_err, (size_t)g->C * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g->d_emax, sizeof(double));
+        if (e == cudaSuccess) e = cudaMallocHost((void **)&g->h_emax, sizeof(double));
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(integrate)");
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    double *cur = rho_dust, *alt = g->trial_rho;        // state ping-pong; the FSAL buffers swap with it
+    double t = 0.0, dt = dt_try, dt_last = 0.0, err_last = 0.0;
+    int n_acc = 0, n_rej = 0, status = CUDISC_OK;
+    while (t < t_span && n_acc + n_rej < max_steps) {
+        const double left = t_span - t;
+        const bool cut = dt >= left;
+        const double h = cut ? left : dt;
+        StepArgs sa;
+        memset(&sa, 0, sizeof(sa));
+        sa.rho = cur; sa.rho_out = alt;
+        sa.k_fsal = g->k_fsal; sa.k_out = g->trial_k;
+        sa.err = g->trial_err;
+        sa.dt = h; sa.rtol = b->p.rtol; sa.atol_factor = b->p.atol_factor;
+        sa.have_k1 = g->fsal_valid ? 1 : 0;
+        rc = run(g, 3, gas_args(g->gs, b->p), sa, stream);
+        if (rc) return rc;
+        e = launch_err_max(g->trial_err, g->C, g->d_emax, st);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(g->h_emax, g->d_emax, sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "integrate step");
+        const double E = *g->h_emax;
+        if (!(E == E) || std::isinf(E)) {
+            status = fail(CUDISC_ERR_INVALID, "non-finite error norm at t = %g s (dt = %g s)", t, h);
+            break;
+        }
+        if (E <= 1.0) {                                 // accept
+            std::swap(cur, alt);
+            std::swap(g->k_fsal, g->trial_k);
+            g->fsal_valid = true;
+            t = cut ? t_span : t + h;
+            dt_last = h; err_last = E;
+            if (dt_log) dt_log[n_acc + n_rej] = h;
+            ++n_acc;
+            const double sug = cudisc_controller_next_dt(E, h);
+            dt = cut ? std::max(sug, dt) : sug;         // a step cut to land on t_span does not shrink dt
+        } else {                                        // reject: state and FSAL buffer untouched
+            if (dt_log) dt_log[n_acc + n_rej] = -h;
+            ++n_rej;
+            dt = cudisc_controller_next_dt(E, h);
+        }
+    }
+    if (cur != rho_dust) {
+        e = cudaMemcpyAsync(rho_dust, cur, row_bytes, cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "integrate copy-back");
+    }
+    if (info) {
+        info->t_done = t; info->dt_last = dt_last; info->dt_next = dt; info->err_last = err_last;
+        info->n_accepted = n_acc; info->n_rejected = n_rej;
+    }
+    return status;
 }
 
 int cudisc_microbench_dfma(int n_iter, double *dfma_per_s, double *elapsed_ms)

@@ -564,6 +564,22 @@ __global__ void __launch_bounds__(256) copy_peak_kernel(const double2 *__restric
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) dst[q] = src[q];
 }
 
+// global error norm of a step: max over cells, NaN wins (one block; C doubles are L2-resident)
+__global__ void __launch_bounds__(1024) err_max_kernel(const double *__restrict__ err, int n, double *out)
+{
+    __shared__ double red[64];
+    double v = 0.0;
+    for (int q = threadIdx.x; q < n; q += 1024) v = nanmax(v, err[q]);
+    v = block_nanmax<1024>(v, red, threadIdx.x);
+    if (threadIdx.x == 0) out[0] = v;
+}
+
+cudaError_t launch_err_max(const double *err, int n, double *out, cudaStream_t st)
+{
+    err_max_kernel<<<1, 1024, 0, st>>>(err, n, out);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_dfma_peak(int grid, int n_iter, double *out, cudaStream_t st)
 {
     dfma_peak_kernel<<<grid, 256, 0, st>>>(out, n_iter, 0.999999, 1e-6);

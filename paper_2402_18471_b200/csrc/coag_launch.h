@@ -19,5 +19,7 @@ cudaError_t launch_cells(int mode, const LaunchCfg &lc, const DevTables &tb, con
 int cells_occupancy(int smem_bytes, int smem_optin);
 cudaError_t launch_dfma_peak(int grid, int n_iter, double *out, cudaStream_t st);
 cudaError_t launch_copy_peak(int grid, const void *src, void *dst, size_t n16, cudaStream_t st);
+// out[0] = NaN-propagating max of err[0..n)
+cudaError_t launch_err_max(const double *err, int n, double *out, cudaStream_t st);
 
 }  // namespace cudisc
