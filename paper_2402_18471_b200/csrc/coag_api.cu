@@ -144,7 +144,7 @@ int upload_tables(cudisc_bins b)
     // ---- eval items: row / column passes, heaviest first.  Partial sums go to packed slots:
     //      row chunk c holds rows i >= rowFirst[c], column range r holds columns j < R1[r]
     const int nchRow = std::min(8, std::max(1, (N + kRowChunk - 1) / kRowChunk));
-    const int nRng = std::min(8, std::max(1, (N + 31) / 32));
+    const int nRng = std::min(8, std::max(1, (N + 63) / 64));
     const int rngLen = (N + nRng - 1) / nRng;
     std::vector<int> sched(kSched, 0);
     int rowSlots = 0, colSlots = 0;

@@ -152,6 +152,9 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         }
     }
 #endif
+#ifdef CUDISC_NOBAND
+    if (false)
+#endif
     for (;;) {
         const int it = next_item(&s.CTR[1], lane);
         if (it >= tb.nEvalItems) break;
@@ -449,6 +452,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
         // ---------------- Bogacki-Shampine 3(2), PAPER.md:478 (tableau: Bogacki & Shampine 1989)
         const double h = sa.dt;
         double k2 = 0.0, k3 = 0.0, k4 = 0.0, yn = y0;
+        PROF_T(tst);
 #pragma unroll 1
         for (int st = sa.have_k1 ? 1 : 0; st < 4; ++st) {
             double ys = y0;
@@ -469,6 +473,8 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
             if (st == 3) k4 = d;
         }
 
+        PROF_ADD(8, tst);
+        PROF_T(ttail);
         // error norm (R10) and write-back
         const double atol = sa.atol_factor * block_sum<NT>(y0, s.RED + 48, tid);
         double emax = 0.0;
@@ -481,6 +487,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
         }
         emax = block_nanmax<NT>(emax, s.RED + 48, tid);
         if (tid == 0) sa.err[cell] = emax;
+        PROF_ADD(7, ttail);
         PROF_ADD(6, tc0);
     }
     if (use_tmem) {
