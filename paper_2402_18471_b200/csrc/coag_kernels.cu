@@ -242,11 +242,15 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     PROF_ADD(4, tpA);
     PROF_T(tpB);
 
-    // ---- phase B (thread <-> bin): combine partials in fixed order
-    double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, G = 0.0, sv = 0.0;
+    // ---- phase B: combine partials in fixed order.  Two warp groups work side by side:
+    //   group R (thread k, bin k)            row partials -> deposits into bins k-1, k, k+1
+    //   group C (thread k + 32 nw, bin k)    column partials -> loss frequency G_k, fragment source,
+    //                                        warp suffix scan of S_l / B_l (Eq. 67 via l-bins)
+    // and meet at one barrier; G_k and the scanned value travel through NN[k] and YY[k].y, dead by now.
+    const int nw = (N + 31) >> 5;
+    double d0 = 0.0, dm1 = 0.0, dp1 = 0.0;
     if (live) {
-        const int2 bi = s.BINI[k];
-        const int nch = ((bi.x & 0x1ff) + kRowChunk - 1) / kRowChunk;
+        const int nch = ((s.BINI[k].x & 0x1ff) + kRowChunk - 1) / kRowChunk;
         double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0;
         for (int c = 0; c < nch; ++c) {
             const double2 *pp = reinterpret_cast<const double2 *>(s.PARTR)
@@ -259,43 +263,54 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         dm1 = nk * (bc[BC_G1 * Np] * f1 - cF2 * f2);
         d0 = nk * ((bc[BC_A1 * Np] * a1 + cA2 * a2) + (bc[BC_F1 * Np] * f1 + cF2 * f2));
         dp1 = nk * (bc[BC_B1 * Np] * a1 - cA2 * a2);
-        // column sums of bin j over the row ranges that hold rows >= j (fixed order)
-        auto colsum = [&](int j, int rfirst, double &gj, double &hj) {
-            gj = 0.0; hj = 0.0;
-            for (int r = rfirst; r < tb.nRng; ++r) {
-                const double2 u = reinterpret_cast<const double2 *>(s.PARTC)[s.SCHED[SC_COLOFF + r] + j];
-                gj += u.x; hj += u.y;
-            }
-        };
-        double gc, h;
-        colsum(k, bi.x >> 18, gc, h);
-        G = gc + h;
-        // fragment source of l-bin k, scaled by 1/B_k
-        double sl = s.BANDV[N + k] + s.BANDV[2 * Np + N + k];
-        for (int j = bi.y & 0xffff; j < (bi.y >> 16); ++j) {
-            double gj, hj = h;
-            if (j != k) colsum(j, s.BINI[j].x >> 18, gj, hj);
-            sl = fma(tb.sS * s.YY[j].x, hj, sl);
-        }
-        sv = sl * bc[BC_FIB * Np];
-    }
-    // inclusive suffix sum over bins (Eq. 67 via the l-bin algorithm): within the warp, then across
-    double suf = sv;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const double v = __shfl_down_sync(0xffffffffu, suf, o);
-        if (lane + o < 32) suf += v;
     }
     double *wtot = s.RED, *eUp = s.RED + 16, *eDn = s.RED + 32;
-    if (lane == 0) { wtot[warp] = suf; eDn[warp] = dm1; }
-    if (lane == 31) eUp[warp] = dp1;
+    if (warp < nw) {
+        if (lane == 0) eDn[warp] = dm1;
+        if (lane == 31) eUp[warp] = dp1;
+    }
     const double up = __shfl_up_sync(0xffffffffu, dp1, 1);
     const double dn = __shfl_down_sync(0xffffffffu, dm1, 1);
+    if (warp >= nw && warp < 2 * nw) {
+        const int kc = tid - 32 * nw;                      // bin of this group-C thread
+        double sv = 0.0;
+        if (kc < N) {
+            const int2 bi = s.BINI[kc];
+            // column sums of bin j over the row ranges that hold rows >= j (fixed order)
+            auto colsum = [&](int j, int rfirst, double &gj, double &hj) {
+                gj = 0.0; hj = 0.0;
+                for (int r = rfirst; r < tb.nRng; ++r) {
+                    const double2 u = reinterpret_cast<const double2 *>(s.PARTC)[s.SCHED[SC_COLOFF + r] + j];
+                    gj += u.x; hj += u.y;
+                }
+            };
+            double gc, h;
+            colsum(kc, bi.x >> 18, gc, h);
+            s.NN[kc] = gc + h;                             // G_k
+            // fragment source of l-bin k, scaled by 1/B_k
+            double sl = s.BANDV[N + kc] + s.BANDV[2 * Np + N + kc];
+            for (int j = bi.y & 0xffff; j < (bi.y >> 16); ++j) {
+                double gj, hj = h;
+                if (j != kc) colsum(j, s.BINI[j].x >> 18, gj, hj);
+                sl = fma(tb.sS * s.YY[j].x, hj, sl);
+            }
+            sv = sl * s.BINC[BC_FIB * Np + kc];
+        }
+        // inclusive suffix sum over the bins of the warp; the warp totals are added after the barrier
+        double suf = sv;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double v = __shfl_down_sync(0xffffffffu, suf, o);
+            if (lane + o < 32) suf += v;
+        }
+        if (lane == 0) wtot[warp - nw] = suf;
+        if (kc < N) s.YY[kc].y = suf;
+    }
     __syncthreads();
 
     double d = 0.0;
     if (live) {
-        const int nw = (N + 31) >> 5;
+        double suf = s.YY[k].y;
         for (int w = warp + 1; w < nw; ++w) suf += wtot[w];
         const double prev = (lane > 0) ? up : (warp > 0 ? eUp[warp - 1] : 0.0);
         const double next = (lane < 31) ? dn : (warp + 1 < nw ? eDn[warp + 1] : 0.0);
@@ -303,7 +318,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         if (k > 0) d += prev;
         if (k < N - 1) d += next;
         d += s.BANDV[k] + s.BANDV[2 * Np + k];
-        d = fma(-y, G, d);
+        d = fma(-y, s.NN[k], d);
         d = fma(s.BINC[BC_FA * Np + k], suf, d);
     }
     PROF_ADD(5, tpB);
