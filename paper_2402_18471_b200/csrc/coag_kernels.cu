@@ -500,7 +500,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
             sa.rho_out[row + k] = yn;
             sa.k_out[row + k] = k4;
         }
-        emax = block_nanmax<NT>(emax, s.RED + 48, tid);
+        emax = block_nanmax<NT>(emax, s.RED + 64, tid);
         if (tid == 0) sa.err[cell] = emax;
         PROF_ADD(7, ttail);
         PROF_ADD(6, tc0);
@@ -592,7 +592,7 @@ __global__ void __launch_bounds__(1024) err_max_kernel(const double *__restrict_
     __shared__ double red[64];
     double v = 0.0;
     for (int q = threadIdx.x; q < n; q += 1024) v = nanmax(v, err[q]);
-    v = block_nanmax<1024>(v, red, threadIdx.x);
+    v = block_nanmax<1024>(v, red, threadIdx.x);   // 32 warps -> 32 slots
     if (threadIdx.x == 0) out[0] = v;
 }
 
