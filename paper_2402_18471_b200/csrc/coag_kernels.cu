@@ -25,8 +25,12 @@ __device__ __forceinline__ void build_items(const DevTables &tb, const Smem &s, 
                                             const PairConst &pc, double *kout, int lane)
 {
     const int N = tb.N, P = tb.P;
+    // the first item of every warp is fixed (item = warp; the counter starts at the warp count):
+    // no pile-up of all warps on one shared-memory atomic at the start of the phase
+    bool first = true;
     for (;;) {
-        const int it = next_item(&s.CTR[0], lane);
+        const int it = first ? (int)(threadIdx.x >> 5) : next_item(&s.CTR[0], lane);
+        first = false;
         if (it >= tb.nBuildItems) break;
         const uint32_t item = s.ITB[it];
         const int c = (item >> 28) & 7, ia = (item >> 14) & 0x3fff, ib = item & 0x3fff;
@@ -110,7 +114,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         s.BANDV[2 * Np + k] = 0.0;                 // second band slot: only split groups write it
         s.BANDV[2 * Np + N + k] = 0.0;
     }
-    if (tid == 0) s.CTR[1] = 0;
+    if (tid == 0) s.CTR[1] = NT / 32;
     __syncthreads();
     PROF_ADD(2, tp0);
     PROF_T(tpA);
@@ -155,8 +159,10 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
 #ifdef CUDISC_NOBAND
     if (false)
 #endif
+    bool first = true;
     for (;;) {
-        const int it = next_item(&s.CTR[1], lane);
+        const int it = first ? NT / 32 - 1 - warp : next_item(&s.CTR[1], lane);
+        first = false;
         if (it >= tb.nEvalItems) break;
         const uint32_t item = s.ITE[it];
         const int kind = item >> 30, ix = (item >> 26) & 15, iy = (item >> 23) & 7;
@@ -437,7 +443,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
             if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, s, k);
             prologue_store(tb, rv, nvR, nvZ, nvP, has_vphi, s, k);
             // V_g^2 through shared memory: only the bin-owning warps hold the pre-computed values
-            if (tid == 0) { s.CTR[0] = 0; reinterpret_cast<double *>(s.CTR)[1] = rv.Vg2; }
+            if (tid == 0) { s.CTR[0] = NT / 32; reinterpret_cast<double *>(s.CTR)[1] = rv.Vg2; }
             __syncthreads();
             pc.Vg2 = reinterpret_cast<const double *>(s.CTR)[1];
             PROF_ADD(0, tc0);
