@@ -230,53 +230,61 @@ int upload_tables(cudisc_bins b)
     }
     d.bandW = W; d.bandL = L;
     // band tables in tensor memory when they fit: target group g sits in the tensor-memory lanes of
-    // quarter g % 4 (columns 128 (g / 4) ...), readable by warps w with w % 4 == g % 4.  Its entry
-    // list is cut into tasks of <= kBandTask entries, dealt to the least loaded warp of the quarter;
-    // a group cut in two sums into the two BANDV slots.
+    // quarter g % 4 (columns 128 (g / 4) ...), readable by warps w with w % 4 == g % 4: its gather
+    // is a task of the least loaded warp of that quarter.
+    //   bandD > 0 (band pairs within bandD of the diagonal and the stage fits): the products
+    //     n_i n_j K of the band pairs are staged once per evaluation (W items) and the indices address
+    //     the stage: plane * bandD * Np + (i - j) * Np + i;
+    //   bandD == 0: indices address the K store; a long list is cut in two tasks (two BANDV slots).
     const int nGroups = (2 * N + 31) / 32;
     d.bandLp = (L + 7) & ~7;
     d.bandTmem = (d.bandLp <= kBandTmemMax && nGroups <= kThreads / 32) ? 1 : 0;
+    int bandD = 0;
+    for (const BandEntry &be : t.band) bandD = std::max(bandD, be.i - be.j + 1);
+    if (!d.bandTmem || t.band.empty() || (size_t)2 * bandD * d.Np * sizeof(double) > 16384) bandD = 0;
     std::vector<uint32_t> evalItems;
     {
         constexpr int nWarps = kThreads / 32;
         int load[nWarps] = {0}, ntask[nWarps] = {0};
         // the bin-owning warps also compute the next cell's per-bin values during the last evaluation
         for (int w = 0; w < nWarps; ++w) load[w] = (32 * w < N) ? 12 : 0;
-        for (int tg = 0; tg < nGroups; ++tg) {
+        for (int tg = 0; tg < nGroups && d.bandTmem; ++tg) {
             int cmax = 0;
             for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
-            if (!d.bandTmem) { evalItems.push_back(pack_eval(IT_BAND, tg, 0, 0, cmax)); continue; }
-            const int Lg = (cmax + 7) & ~7;
-            if (Lg == 0) continue;   // phase 0 does not zero slot 0: every group with targets needs a task
-        }
-        if (d.bandTmem) {
-            for (int tg = 0; tg < nGroups; ++tg) {
-                int cmax = 0;
-                for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
-                const int Lg = (cmax + 7) & ~7;
-                const int half = (Lg > 16) ? ((Lg / 2 + 7) & ~7) : Lg;
-                const int cuts[3] = {0, half, Lg};
-                for (int h = 0; h < 2; ++h) {
-                    if (h == 1 && cuts[1] == cuts[2]) break;
-                    int best = -1;
-                    for (int w = tg % 4; w < nWarps; w += 4)
-                        if (ntask[w] < 2 && (best < 0 || load[w] < load[best])) best = w;
-                    if (best < 0) { d.bandTmem = 0; break; }
-                    sched[SC_BTASK + 2 * best + ntask[best]] =
-                        (int)(0x80000000u | ((uint32_t)h << 30) | ((uint32_t)tg << 16) |
-                              ((uint32_t)cuts[h] << 8) | (uint32_t)cuts[h + 1]);
-                    ntask[best]++;
-                    load[best] += cuts[h + 1] - cuts[h] + 4;
-                }
+            const int Lg = (cmax + 7) & ~7;        // a group without entries still gets a task: it zeroes BANDV
+            const int half = (!bandD && Lg > 16) ? ((Lg / 2 + 7) & ~7) : Lg;
+            const int cuts[3] = {0, half, Lg};
+            for (int h = 0; h < 2; ++h) {
+                if (h == 1 && cuts[1] == cuts[2]) break;
+                int best = -1;
+                for (int w = tg % 4; w < nWarps; w += 4)
+                    if (ntask[w] < 2 && (best < 0 || load[w] < load[best])) best = w;
+                if (best < 0) { d.bandTmem = 0; break; }
+                sched[SC_BTASK + 2 * best + ntask[best]] =
+                    (int)(0x80000000u | ((uint32_t)h << 30) | ((uint32_t)tg << 16) |
+                          ((uint32_t)cuts[h] << 8) | (uint32_t)cuts[h + 1]);
+                ntask[best]++;
+                load[best] += cuts[h + 1] - cuts[h] + 4;
             }
         }
-        if (!d.bandTmem && evalItems.empty())
+        if (!d.bandTmem) {
+            bandD = 0;
+            for (int q = 0; q < 2 * nWarps; ++q) sched[SC_BTASK + q] = 0;
             for (int tg = 0; tg < nGroups; ++tg) {
                 int cmax = 0;
                 for (int q = tg * 32; q < std::min(W, tg * 32 + 32); ++q) cmax = std::max(cmax, cnt[q]);
                 evalItems.push_back(pack_eval(IT_BAND, tg, 0, 0, cmax));
             }
-        if (!d.bandTmem) for (int q = 0; q < 2 * nWarps; ++q) sched[SC_BTASK + q] = 0;
+        }
+    }
+    d.bandD = bandD; d.nWItems = 0;
+    if (bandD) {
+        for (uint32_t &ix : bidx) {                 // padding entries (coef 0) point at stage slot 0
+            const int i = ix & 0xff, j = (ix >> 8) & 0xff, plane = (ix >> 16) & 1;
+            ix = (uint32_t)(plane * bandD * d.Np + (i - j) * d.Np + i);
+        }
+        for (int blk = 0; blk < nblk; ++blk) evalItems.push_back(pack_eval(IT_W, blk, 0, 0, 0));
+        d.nWItems = nblk;
     }
     for (const Cost &c : work) evalItems.push_back(c.item);
     d.nBuildItems = (int)buildItems.size(); d.nEvalItems = (int)evalItems.size();
@@ -452,7 +460,7 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
     g->num_sms = sms; g->smem_optin = optin;
 
     const DevTables &d = b->dt;
-    const size_t vec_bytes = smem_vec_doubles(d.Np, d.partRowSlots, d.partColSlots, d.nBuildItems + d.nEvalItems) * sizeof(double);
+    const size_t vec_bytes = smem_vec_doubles(d.Np, d.partRowSlots, d.partColSlots, d.nBuildItems + d.nEvalItems, d.bandD) * sizeof(double);
     if (vec_bytes + 16 * 64 > (size_t)optin) {
         delete g;
         return fail(CUDISC_ERR_UNSUPPORTED, "n_bins %d needs %zu B of shared memory", d.N, vec_bytes);

@@ -111,10 +111,12 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         nk = y * s.BINC[BC_RM * Np + k];
         s.NN[k] = nk;
         s.YY[k] = make_double2(y, y * s.BINC[BC_M * Np + k]);
-        s.BANDV[2 * Np + k] = 0.0;                 // second band slot: only split groups write it
-        s.BANDV[2 * Np + N + k] = 0.0;
+        if (!tb.bandD) {                           // second band slot: only split groups write it
+            s.BANDV2[k] = 0.0;
+            s.BANDV2[N + k] = 0.0;
+        }
     }
-    if (tid == 0) s.CTR[1] = NT / 32;
+    if (tid == 0) { s.CTR[1] = NT / 32; s.CTR[2] = 0; }
     __syncthreads();
     PROF_ADD(2, tp0);
     PROF_T(tpA);
@@ -127,7 +129,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     //      tensor-memory lanes of its quarter), then row sums, column sums (and, without
     //      tensor-memory tables, band gathers) pulled by warps
 #ifndef CUDISC_NOBAND
-    if (tb.bandTmem) {
+    if (tb.bandTmem && !tb.bandD) {
 #pragma unroll 1
         for (int q = 0; q < 2; ++q) {
             const int task = s.SCHED[SC_BTASK + 2 * warp + q];
@@ -152,13 +154,43 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
                     else acc0 = fma(c * s.NN[i], s.NN[j] * kv, acc0);
                 }
             }
-            if (t < 2 * N) s.BANDV[((task >> 30) & 1) * 2 * Np + t] = acc0 + acc1;
+            if (t < 2 * N) (((task >> 30) & 1) ? s.BANDV2 : s.BANDV)[t] = acc0 + acc1;
         }
     }
 #endif
 #ifdef CUDISC_NOBAND
     if (false)
 #endif
+    // band gathers from the staged products (tensor-memory coefficients and stage indices): run by the
+    // owning warp after its first item, when the (short, first-claimed) W items are done
+    auto band_from_stage = [&]() {
+#pragma unroll 1
+        for (int q = 0; q < 2; ++q) {
+            const int task = s.SCHED[SC_BTASK + 2 * warp + q];
+            if (task >= 0) break;                                  // valid bit = sign bit
+            while (*reinterpret_cast<volatile int *>(&s.CTR[2]) < tb.nWItems) { }
+            __threadfence_block();
+            const int g = (task >> 16) & 0xff, e0b = (task >> 8) & 0xff, e1b = task & 0xff;
+            const int t = 32 * g + lane, Lp = tb.bandLp;
+            const uint32_t tc = tmem_warp_addr(tbase, g, 0), ti = tc + 2 * Lp;
+            double acc0 = 0.0, acc1 = 0.0;
+            for (int e0 = e0b; e0 < e1b; e0 += 8) {
+                uint32_t cf[16], ixs[8];
+                tmem_ld16(tc + 2 * e0, cf);
+                tmem_ld8(ti + e0, ixs);
+                tmem_wait_ld();
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const double c = __hiloint2double((int)cf[2 * u + 1], (int)cf[2 * u]);
+                    if (u & 1) acc1 = fma(c, s.WST[ixs[u]], acc1);
+                    else acc0 = fma(c, s.WST[ixs[u]], acc0);
+                }
+            }
+            if (t < 2 * N) s.BANDV[t] = acc0 + acc1;
+        }
+    };
+    const bool stage_band = tb.bandTmem && tb.bandD && s.SCHED[SC_BTASK + 2 * warp] < 0;
+    bool band_done = !stage_band;
     bool first = true;
     for (;;) {
         const int it = first ? NT / 32 - 1 - warp : next_item(&s.CTR[1], lane);
@@ -222,6 +254,22 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
                 }
                 reinterpret_cast<double2 *>(s.PARTC)[s.SCHED[SC_COLOFF + iy] + j] = make_double2(gc + gc2, h + h2);
             }
+        } else if (kind == IT_W) {
+            // band products of rows i = 32 ix + lane: W[d][i] = n_i n_{i-d} (K p_coag, K p_frag), d < bandD
+            const int i = 32 * ix + lane;
+            if (i < N) {
+                const double ni = s.NN[i];
+                const int base = tri(i);
+                double *wc = s.WST + i, *wf = wc + (size_t)tb.bandD * Np;
+                for (int dd = 0; dd < tb.bandD && dd <= i; ++dd) {
+                    const double2 k2 = ks.ld(base + i - dd);
+                    const double w = ni * s.NN[i - dd];
+                    wc[dd * Np] = w * k2.x;
+                    wf[dd * Np] = w * k2.y;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) { __threadfence_block(); atomicAdd(&s.CTR[2], 1); }
         } else {
             // band gather from global tables (fallback): lane <-> target t of group ix
             const int t = 32 * ix + lane;
@@ -239,11 +287,10 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
             }
             if (t < 2 * N) s.BANDV[t] = acc;
         }
+        if (!band_done) { band_from_stage(); band_done = true; }
     }
+    if (!band_done) band_from_stage();
     PROF_ADD(3, tpA);
-#ifdef CUDISC_PROF
-    if (lane == 0) sa_prof[16 + warp] += clock64() - tpA;
-#endif
     __syncthreads();
     PROF_ADD(4, tpA);
     PROF_T(tpB);
@@ -294,7 +341,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
             colsum(kc, bi.x >> 18, gc, h);
             s.NN[kc] = gc + h;                             // G_k
             // fragment source of l-bin k, scaled by 1/B_k
-            double sl = s.BANDV[N + kc] + s.BANDV[2 * Np + N + kc];
+            double sl = s.BANDV[N + kc] + (tb.bandD ? 0.0 : s.BANDV2[N + kc]);
             for (int j = bi.y & 0xffff; j < (bi.y >> 16); ++j) {
                 double gj, hj = h;
                 if (j != kc) colsum(j, s.BINI[j].x >> 18, gj, hj);
@@ -323,7 +370,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         d = d0;
         if (k > 0) d += prev;
         if (k < N - 1) d += next;
-        d += s.BANDV[k] + s.BANDV[2 * Np + k];
+        d += s.BANDV[k] + (tb.bandD ? 0.0 : s.BANDV2[k]);
         d = fma(-y, s.NN[k], d);
         d = fma(s.BINC[BC_FA * Np + k], suf, d);
     }
@@ -342,8 +389,8 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
     ks.sm = reinterpret_cast<double2 *>(smem_raw);
     ks.Psm = sa.Psm;
     ks.gl = reinterpret_cast<double2 *>(sa.kslab) + (size_t)blockIdx.x * (size_t)(P - sa.Psm);
-    const Smem s = carve(smem_raw + 2 * (size_t)sa.Psm, tb.Np, tb.partRowSlots, tb.nBuildItems,
-                         tb.nEvalItems);
+    const Smem s = carve(smem_raw + 2 * (size_t)sa.Psm, tb.Np, tb.partRowSlots, tb.partColSlots,
+                         tb.nBuildItems, tb.nEvalItems, tb.bandD);
     PairConst pc;
     const bool has_vphi = gs.vphi != nullptr;
     pc.c15vf2 = 1.5 * gs.v_frag * gs.v_frag;
@@ -443,9 +490,9 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
             if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, s, k);
             prologue_store(tb, rv, nvR, nvZ, nvP, has_vphi, s, k);
             // V_g^2 through shared memory: only the bin-owning warps hold the pre-computed values
-            if (tid == 0) { s.CTR[0] = NT / 32; reinterpret_cast<double *>(s.CTR)[1] = rv.Vg2; }
+            if (tid == 0) { s.CTR[0] = NT / 32; s.RED[95] = rv.Vg2; }
             __syncthreads();
-            pc.Vg2 = reinterpret_cast<const double *>(s.CTR)[1];
+            pc.Vg2 = s.RED[95];
             PROF_ADD(0, tc0);
         }
         // state (thread <-> bin): in flight during the build
