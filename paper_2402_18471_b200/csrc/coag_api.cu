@@ -143,8 +143,8 @@ int upload_tables(cudisc_bins b)
 
     // ---- eval items: row / column passes, heaviest first.  Partial sums go to packed slots:
     //      row chunk c holds rows i >= rowFirst[c], column range r holds columns j < R1[r]
-    const int nchRow = std::min(8, std::max(1, (N + kRowChunk - 1) / kRowChunk));
-    const int nRng = std::min(8, std::max(1, (N + 63) / 64));
+    const int nchRow = std::min(4, std::max(1, (N + kRowChunk - 1) / kRowChunk));
+    const int nRng = std::min(4, std::max(1, (N + 63) / 64));
     const int rngLen = (N + nRng - 1) / nRng;
     std::vector<int> sched(kSched, 0);
     int rowSlots = 0, colSlots = 0;
@@ -161,6 +161,10 @@ int upload_tables(cudisc_bins b)
         colSlots += std::min(N, (r + 1) * rngLen);
     }
     d.partRowSlots = rowSlots; d.partColSlots = colSlots;
+    for (int c = 0; c < 4; ++c) {
+        d.rowBase[c] = c < nchRow ? sched[SC_ROWOFF + c] - sched[SC_ROWFIRST + c] : 0;
+        d.colOff[c] = c < nRng ? sched[SC_COLOFF + c] : 0;
+    }
     struct Cost { uint32_t item; long cost; };
     std::vector<Cost> work;
     for (int blk = 0; blk < nblk; ++blk)

@@ -225,7 +225,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
             }
             const int first = s.SCHED[SC_ROWFIRST + iy];
             if (i < N && i >= first) {
-                double2 *pp = reinterpret_cast<double2 *>(s.PARTR) + 2 * (s.SCHED[SC_ROWOFF + iy] + i - first);
+                double2 *pp = reinterpret_cast<double2 *>(s.PARTR) + 2 * (s.SCHED[SC_ROWOFF + iy] - first + i);
                 pp[0] = make_double2(a1 + b1, a2 + b2);
                 pp[1] = make_double2(f1 + g1, f2 + g2);
             }
@@ -303,13 +303,16 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     const int nw = (N + 31) >> 5;
     double d0 = 0.0, dm1 = 0.0, dp1 = 0.0;
     if (live) {
-        const int nch = ((s.BINI[k].x & 0x1ff) + kRowChunk - 1) / kRowChunk;
+        const int nb = s.BINI[k].x & 0x1ff;
         double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0;
-        for (int c = 0; c < nch; ++c) {
-            const double2 *pp = reinterpret_cast<const double2 *>(s.PARTR)
-                                + 2 * (s.SCHED[SC_ROWOFF + c] + k - s.SCHED[SC_ROWFIRST + c]);
-            const double2 u = pp[0], v = pp[1];
-            a1 += u.x; a2 += u.y; f1 += v.x; f2 += v.y;
+        // (straight-line: slot bases are kernel constants, the loads of all chunks issue together)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            if (nb > kRowChunk * c) {
+                const double2 *pp = reinterpret_cast<const double2 *>(s.PARTR) + 2 * (tb.rowBase[c] + k);
+                const double2 u = pp[0], v = pp[1];
+                a1 += u.x; a2 += u.y; f1 += v.x; f2 += v.y;
+            }
         }
         const double *bc = s.BINC + k;
         const double cA2 = bc[BC_A2 * Np], cF2 = bc[BC_F2 * Np];
@@ -332,9 +335,12 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
             // column sums of bin j over the row ranges that hold rows >= j (fixed order)
             auto colsum = [&](int j, int rfirst, double &gj, double &hj) {
                 gj = 0.0; hj = 0.0;
-                for (int r = rfirst; r < tb.nRng; ++r) {
-                    const double2 u = reinterpret_cast<const double2 *>(s.PARTC)[s.SCHED[SC_COLOFF + r] + j];
-                    gj += u.x; hj += u.y;
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    if (r >= rfirst && r < tb.nRng) {
+                        const double2 u = reinterpret_cast<const double2 *>(s.PARTC)[tb.colOff[r] + j];
+                        gj += u.x; hj += u.y;
+                    }
                 }
             };
             double gc, h;
