@@ -484,13 +484,28 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
 
         // ---------------- K store for this cell
         if (MODE == MODE_RATES) {
+            // flat, coalesced copy of both planes (8 loads in flight per thread), then the N diagonal
+            // entries are halved in place
             const double *k0 = sa.Kin + (size_t)cell * 2 * P, *k1 = k0 + P;
-            for (int i = tid >> 5; i < N; i += NT / 32) {
-                const int base = tri(i);
-                for (int j = lane; j <= i; j += 32) {
-                    const double h = (i == j) ? 0.5 : 1.0;
-                    ks.st(base + j, make_double2(h * __ldg(k0 + base + j), h * __ldg(k1 + base + j)));
+            for (int p0 = tid; p0 < P; p0 += 4 * NT) {
+                double a[4], b[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int p = p0 + u * NT;
+                    a[u] = p < P ? __ldcs(k0 + p) : 0.0;
+                    b[u] = p < P ? __ldcs(k1 + p) : 0.0;
                 }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int p = p0 + u * NT;
+                    if (p < P) ks.st(p, make_double2(a[u], b[u]));
+                }
+            }
+            __syncthreads();
+            if (live) {
+                const int p = tri(k) + k;
+                const double2 v = ks.ld(p);
+                ks.st(p, make_double2(0.5 * v.x, 0.5 * v.y));
             }
         } else {
             if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, s, k);
