@@ -130,7 +130,7 @@ int upload_tables(cudisc_bins b)
 
     // ---- build items (all about equal: small items for balance), packed (coag_device.cuh)
     std::vector<uint32_t> buildItems;
-    constexpr int kRowsPerItem = 6, kPairsPerItem = 64;
+    constexpr int kRowsPerItem = 24, kPairsPerItem = 96;
     for (int c = 0; c < nblk; ++c)
         for (int ia = 32 * c + 32; ia < N; ia += kRowsPerItem)
             buildItems.push_back(pack_build(IT_BUILD_ROWS, c, ia, std::min(N, ia + kRowsPerItem)));
