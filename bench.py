@@ -308,8 +308,8 @@ def run_ours(args):
                 "bound": "alu", "kernel": "cudisc::coag_cells_kernel<512, MODE_STEP, false>",
                 "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops,
-                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, profiles/r01_v5_step_kernel.md
-                "traffic": 193147136 if (args.config == 4 and world == 1) else None,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, profiles/r01_v7_step_kernel.md
+                "traffic": 193176832 if (args.config == 4 and world == 1) else None,
                 "how": f"algorithmic FP64 instructions per launch = C*P*({I_BUILD} + {EVALS_PER_STEP}*{I_EVAL}) "
                        f"= {alg_instr:.4g} (DESIGN.md 'Roofline'), x2 flop per FP64 issue slot, / mean CUDA-event "
                        f"launch duration {1e3 * kernel_s:.3f} ms; peak = {sm_count} SMs x {FP64_LANES_PER_SM} "
