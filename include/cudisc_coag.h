@@ -107,6 +107,18 @@ int cudisc_bins_query(cudisc_bins b, int *n_bins, double *m_centres, double *m_e
 int cudisc_bins_expand_outcomes(cudisc_bins b, long long *n_entries, int *target, int *i, int *j,
                                 int *plane, double *coef, double *frag_A, double *frag_invB);
 
+/* Host-side self-check of the work-item schedule the kernels run for this mass grid (no device
+ * needed): decodes the packed items exactly as the device code does and counts what is wrong.
+ *   out[0] pairs (i >= j) not built exactly once by the build items
+ *   out[1] (row i, column j < n_bulk[i]) not summed exactly once by the row-pass items
+ *   out[2] (i >= j) not summed exactly once by the column-pass items
+ *   out[3] partial-sum slots out of range, written twice, or read by the combine step but never written
+ *   out[4] band indices out of range of what they address, or band entries lost
+ *   out[5] band gather tasks: target groups without exactly one covering set of tasks
+ *   out[6] number of items (build + eval);  out[7] shared-memory bytes needed besides the K store
+ * out[0..5] are 0 for a correct schedule.  out: HOST [8]. */
+int cudisc_bins_schedule_check(cudisc_bins b, long long *out);
+
 /* Cell grid of n_r x n_z cells using mass grid b.  Allocates on the current CUDA device: the
  * FSAL buffer [C x N], and the kernel scratch.  The handle remembers b. */
 int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out);

@@ -43,7 +43,7 @@ class cudisc_integrate_info(C.Structure):
 
 EXPORTS = [
     "cudisc_bins_create", "cudisc_bins_create_general", "cudisc_bins_destroy", "cudisc_bins_query",
-    "cudisc_bins_expand_outcomes", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
+    "cudisc_bins_expand_outcomes", "cudisc_bins_schedule_check", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
     "cudisc_grid_destroy", "cudisc_coag_kernel", "cudisc_coag_rates", "cudisc_coag_rates_otf",
     "cudisc_coag_step", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_controller_next_dt",
     "cudisc_microbench_dfma",
@@ -67,6 +67,7 @@ def lib() -> C.CDLL:
         L.cudisc_bins_destroy.argtypes = [vp]
         L.cudisc_bins_query.argtypes = [vp, ip, dp, dp, dp, ip, ip]
         L.cudisc_bins_expand_outcomes.argtypes = [vp, C.POINTER(C.c_longlong), ip, ip, ip, ip, dp, dp, dp]
+        L.cudisc_bins_schedule_check.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.cudisc_grid_create.argtypes = [C.c_int, C.c_int, vp, C.POINTER(vp)]
         L.cudisc_grid_bind_gas.argtypes = [vp, C.POINTER(cudisc_gas_state)]
         L.cudisc_grid_reset_fsal.argtypes = [vp]
@@ -175,6 +176,13 @@ class Bins:
                                              j.ctypes.data_as(ip), pl.ctypes.data_as(ip), coef.ctypes.data_as(dp),
                                              fA.ctypes.data_as(dp), fiB.ctypes.data_as(dp)))
         return {"target": tgt, "i": i, "j": j, "plane": pl, "coef": coef, "frag_A": fA, "frag_invB": fiB}
+
+    def schedule_check(self):
+        """Host-side self-check of the kernels' work-item schedule (no GPU needed): 8 counters, the
+        first six must be zero (include/cudisc_coag.h)."""
+        out = (C.c_longlong * 8)()
+        _check(lib().cudisc_bins_schedule_check(self._h, out))
+        return [int(v) for v in out]
 
     def close(self):
         if self._h:

@@ -111,15 +111,18 @@ struct Blob {
     template <class T> size_t add(const std::vector<T> &v) { return add(v.data(), v.size() * sizeof(T)); }
 };
 
-int upload_tables(cudisc_bins b)
-{
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
-    if (b->on_device && b->device == dev) return CUDISC_OK;
-    if (b->on_device) { cudaFree(b->dev_blob); b->on_device = false; b->dev_blob = nullptr; }
+// Everything the kernels need besides the K store, built on the host from the grid-only tables:
+// work items, packed slot offsets, band ELL / tensor-memory tasks, per-bin constants.  No CUDA calls.
+struct Schedule {
+    DevTables d;                       // scalars only; pointers are set after the upload
+    std::vector<uint32_t> buildItems, evalItems, bidx;
+    std::vector<int> sched, cnt;
+    std::vector<double> binc, bcoef, dtab, exptab;
+    std::vector<int2> bini;
+};
 
-    const HostTables &t = b->ht;
+void build_schedule(const HostTables &t, Schedule &S)
+{
     const int N = t.N;
     DevTables d;
     memset(&d, 0, sizeof(d));
@@ -293,6 +296,30 @@ int upload_tables(cudisc_bins b)
     for (const Cost &c : work) evalItems.push_back(c.item);
     d.nBuildItems = (int)buildItems.size(); d.nEvalItems = (int)evalItems.size();
 
+    S.d = d;
+    S.buildItems = std::move(buildItems); S.evalItems = std::move(evalItems); S.bidx = std::move(bidx);
+    S.sched = std::move(sched); S.cnt = std::move(cnt);
+    S.binc = std::move(binc); S.bcoef = std::move(bcoef); S.dtab = std::move(dtab); S.exptab = std::move(exptab);
+    S.bini = std::move(bini);
+}
+
+int upload_tables(cudisc_bins b)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (b->on_device && b->device == dev) return CUDISC_OK;
+    if (b->on_device) { cudaFree(b->dev_blob); b->on_device = false; b->dev_blob = nullptr; }
+
+    const HostTables &t = b->ht;
+    Schedule S;
+    build_schedule(t, S);
+    DevTables d = S.d;
+    const std::vector<uint32_t> &buildItems = S.buildItems, &evalItems = S.evalItems, &bidx = S.bidx;
+    const std::vector<int> &sched = S.sched, &cnt = S.cnt;
+    const std::vector<double> &binc = S.binc, &bcoef = S.bcoef, &dtab = S.dtab, &exptab = S.exptab;
+    const std::vector<int2> &bini = S.bini;
+
     Blob bl;
     const size_t o_a = bl.add(t.a), o_binc = bl.add(binc), o_bini = bl.add(bini);
     const size_t o_cnt = bl.add(cnt), o_bidx = bl.add(bidx), o_bcoef = bl.add(bcoef);
@@ -434,6 +461,128 @@ int cudisc_bins_expand_outcomes(cudisc_bins b, long long *n_entries, int *target
     }
     if (frag_A) memcpy(frag_A, b->ht.fA.data(), sizeof(double) * b->ht.N);
     if (frag_invB) memcpy(frag_invB, b->ht.finvB.data(), sizeof(double) * b->ht.N);
+    return CUDISC_OK;
+}
+
+int cudisc_bins_schedule_check(cudisc_bins b, long long *out)
+{
+    if (!bins_ok(b)) return fail(CUDISC_ERR_HANDLE, "bad bins handle");
+    if (!out) return fail(CUDISC_ERR_INVALID, "out is NULL");
+    const HostTables &t = b->ht;
+    Schedule S;
+    build_schedule(t, S);
+    const DevTables &d = S.d;
+    const int N = d.N, Np = d.Np;
+    long long bad[6] = {0, 0, 0, 0, 0, 0};
+    auto tri_h = [](int i) { return i * (i + 1) / 2; };
+    // ---- build items
+    std::vector<int> built((size_t)N * N, 0);
+    for (uint32_t item : S.buildItems) {
+        const int c = (item >> 28) & 7, ia = (item >> 14) & 0x3fff, ib = item & 0x3fff;
+        if ((item >> 31) == IT_BUILD_ROWS) {
+            for (int i = ia; i < ib; ++i)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const int j = 32 * c + lane;
+                    if (j >= N) continue;
+                    if (i >= N || j >= i) { ++bad[0]; continue; }      // rows items never hold the diagonal
+                    built[(size_t)i * N + j]++;
+                }
+        } else {
+            for (int tt = ia; tt < ib; ++tt) {
+                int r = (int)((std::sqrt(8.0 * tt + 1.0) - 1.0) * 0.5);
+                while (tri_h(r + 1) <= tt) ++r;
+                while (tri_h(r) > tt) --r;
+                const int i = 32 * c + r, j = 32 * c + (tt - tri_h(r));
+                if (i >= N || j > i) { ++bad[0]; continue; }
+                built[(size_t)i * N + j]++;
+            }
+        }
+    }
+    for (int i = 0; i < N; ++i)
+        for (int j = 0; j <= i; ++j) bad[0] += built[(size_t)i * N + j] != 1;
+    // ---- eval items
+    std::vector<int> rowcov((size_t)N * N, 0), colcov((size_t)N * N, 0);
+    std::vector<int> rowslot(std::max(1, d.partRowSlots), 0), colslot(std::max(1, d.partColSlots), 0);
+    int nW = 0;
+    for (uint32_t item : S.evalItems) {
+        const int kind = item >> 30, ix = (item >> 26) & 15, iy = (item >> 23) & 7;
+        const int iz = (item >> 9) & 0x1ff, iw = item & 0x1ff;
+        if (kind == IT_ROW) {
+            const int first = S.sched[SC_ROWFIRST + iy];
+            for (int lane = 0; lane < 32; ++lane) {
+                const int i = 32 * ix + lane;
+                if (i >= N) continue;
+                const int jb = kRowChunk * iy, je = std::min(jb + kRowChunk, t.n_bulk[i]);
+                for (int j = jb; j < iw; ++j)
+                    if (j < je) rowcov[(size_t)i * N + j]++;
+                if (je > iw) ++bad[1];                                 // host bound too small
+                if (i >= first) {
+                    const int slot = S.sched[SC_ROWOFF + iy] + i - first;
+                    if (slot < 0 || slot >= d.partRowSlots || slot != d.rowBase[iy] + i) ++bad[3];
+                    else if (rowslot[slot]++) ++bad[3];
+                }
+            }
+        } else if (kind == IT_COL) {
+            for (int lane = 0; lane < 32; ++lane) {
+                const int j = 32 * ix + lane;
+                if (j >= std::min(N, iw)) continue;
+                for (int i = std::max(iz, j); i < iw; ++i) colcov[(size_t)i * N + j]++;
+                const int slot = S.sched[SC_COLOFF + iy] + j;
+                if (slot < 0 || slot >= d.partColSlots || slot != d.colOff[iy] + j) ++bad[3];
+                else if (colslot[slot]++) ++bad[3];
+            }
+        } else if (kind == IT_W) {
+            ++nW;
+        }
+    }
+    for (int i = 0; i < N; ++i)
+        for (int j = 0; j <= i; ++j) {
+            bad[1] += rowcov[(size_t)i * N + j] != (j < t.n_bulk[i] ? 1 : 0);
+            bad[2] += colcov[(size_t)i * N + j] != 1;
+        }
+    // slots the combine step (phase B) reads must have been written
+    for (int k = 0; k < N; ++k) {
+        for (int c = 0; c < 4; ++c)
+            if (t.n_bulk[k] > kRowChunk * c && !(c < d.nchRow && rowslot[d.rowBase[c] + k] == 1)) ++bad[3];
+        for (int r = k / d.rngLen; r < d.nRng; ++r)
+            if (colslot[d.colOff[r] + k] != 1) ++bad[3];
+    }
+    // ---- band
+    long long entries = 0;
+    for (int q = 0; q < d.bandW; ++q) entries += S.cnt[q];
+    if (entries != (long long)t.band.size()) ++bad[4];
+    if (d.bandD) {
+        if (nW != d.nWItems || nW != (N + 31) / 32) ++bad[4];
+        for (uint32_t ix : S.bidx)
+            if (ix >= (uint32_t)(2 * d.bandD * Np)) ++bad[4];
+    } else {
+        for (uint32_t ix : S.bidx) {
+            const int i = ix & 0xff, j = (ix >> 8) & 0xff;
+            if (i >= N || j > i) ++bad[4];
+        }
+    }
+    if (d.bandTmem) {
+        const int nGroups = (2 * N + 31) / 32;
+        std::vector<int> covered(nGroups, 0);
+        for (int w = 0; w < kThreads / 32; ++w)
+            for (int q = 0; q < 2; ++q) {
+                const int task = S.sched[SC_BTASK + 2 * w + q];
+                if (task >= 0) continue;
+                const int g = (task >> 16) & 0xff, e0 = (task >> 8) & 0xff, e1 = task & 0xff;
+                if (g >= nGroups || (g & 3) != (w & 3) || e0 > e1 || e1 > d.bandLp || (e0 & 7) || (e1 & 7)) { ++bad[5]; continue; }
+                covered[g] += (e1 - e0) + 1000;                        // entries + one per task
+            }
+        for (int g = 0; g < nGroups; ++g) {
+            int cmax = 0;
+            for (int q = 32 * g; q < std::min(d.bandW, 32 * g + 32); ++q) cmax = std::max(cmax, S.cnt[q]);
+            const int Lg = (cmax + 7) & ~7, ntask = covered[g] / 1000, ent = covered[g] % 1000;
+            if (ntask < 1 || ntask > 2 || ent != Lg) ++bad[5];
+        }
+    }
+    for (int q = 0; q < 6; ++q) out[q] = bad[q];
+    out[6] = (long long)S.buildItems.size() + (long long)S.evalItems.size();
+    out[7] = (long long)(smem_vec_doubles(Np, d.partRowSlots, d.partColSlots, d.nBuildItems + d.nEvalItems, d.bandD)
+                         * sizeof(double));
     return CUDISC_OK;
 }
 

@@ -102,3 +102,31 @@ def test_general_grid_tables_match_log_grid_tables():
     for k in e1:
         np.testing.assert_array_equal(e1[k], e2[k])
     np.testing.assert_allclose(b2.query()["a_centres"], q["a_centres"], rtol=1e-14)
+
+
+@pytest.mark.parametrize("n_bins,a_min,a_max", [(2, 1e-5, 1.0), (3, 1e-5, 1e-3), (31, 1e-5, 1.0), (32, 1e-5, 1.0),
+                                                (33, 1e-5, 10.0), (40, 1e-5, 1.0), (64, 1e-5, 10.0), (65, 1e-5, 10.0),
+                                                (100, 1e-5, 10.0), (135, 1e-5, 20.0), (150, 1e-5, 10.0),
+                                                (200, 1e-6, 100.0), (255, 1e-6, 100.0), (256, 1e-6, 100.0)])
+def test_work_item_schedule_covers_everything_exactly_once(n_bins, a_min, a_max):
+    """The packed work items the kernels run, decoded on the host exactly as the device code does:
+    every pair built once, every bulk (row, column) and every (i >= j) summed once, every partial-sum
+    slot the combine step reads written once, band indices and gather tasks consistent."""
+    b = cd.Bins(n_bins, a_min, a_max, 1.67, cd.Params())
+    out = b.schedule_check()
+    assert out[:6] == [0, 0, 0, 0, 0, 0], out
+    assert out[6] > 0
+    if n_bins <= 150:   # the whole K store of BASELINE.json configs 1-4 stays in shared memory (227 KB opt-in)
+        assert out[7] + 16 * n_bins * (n_bins + 1) // 2 <= 227 * 1024
+
+
+def test_work_item_schedule_general_grid():
+    rng = np.random.default_rng(3)
+    N = 70
+    g = orc.mass_grid(N, 1e-5, 10.0, 1.67)
+    m_e = g.m_e * np.exp(rng.uniform(-0.05, 0.05, N + 1))
+    m_e.sort()
+    m_c = np.sqrt(m_e[:-1] * m_e[1:])
+    b = cd.Bins(N, 0, 0, 1.67, cd.Params(chi_im=2.5), m_centres=m_c, m_edges=m_e)
+    out = b.schedule_check()
+    assert out[:6] == [0, 0, 0, 0, 0, 0], out
