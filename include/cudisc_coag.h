@@ -171,6 +171,14 @@ int cudisc_coag_rates_otf(cudisc_grid g, cudisc_bins b, const double *rho_dust, 
 int cudisc_coag_step(cudisc_grid g, cudisc_bins b, double *rho_dust, double dt,
                      double *err_out, cudisc_stream stream);
 
+/* Cached-kernel form of cudisc_coag_step: the same Bogacki-Shampine 3(2) step with the
+ * kernel read from K (DEVICE [C][2][P], as written by cudisc_coag_kernel; ANY symmetric kernel is
+ * accepted, e.g. the closed-form test kernels with plane 1 = 0) instead of being built from the gas
+ * state.  16 B of HBM traffic per pair and step.  Shares the FSAL buffer with cudisc_coag_step:
+ * call cudisc_grid_reset_fsal when switching between the two or changing K. */
+int cudisc_coag_step_cached(cudisc_grid g, cudisc_bins b, const double *K, double *rho_dust, double dt,
+                            double *err_out, cudisc_stream stream);
+
 /* End-to-end form of cudisc_coag_step for callers whose dust array lives in HOST memory (the
  * other solvers of the paper's global loop, when they run elsewhere):
  * rho_host: HOST [C x N] in/out, err_host: HOST [C] out (page-locked memory makes the copies

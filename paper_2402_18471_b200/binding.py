@@ -45,7 +45,7 @@ EXPORTS = [
     "cudisc_bins_create", "cudisc_bins_create_general", "cudisc_bins_destroy", "cudisc_bins_query",
     "cudisc_bins_expand_outcomes", "cudisc_bins_schedule_check", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
     "cudisc_grid_destroy", "cudisc_coag_kernel", "cudisc_coag_rates", "cudisc_coag_rates_otf",
-    "cudisc_coag_step", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_controller_next_dt",
+    "cudisc_coag_step", "cudisc_coag_step_cached", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_controller_next_dt",
     "cudisc_microbench_dfma",
     "cudisc_microbench_copy", "cudisc_launch_count", "cudisc_last_error", "cudisc_version",
 ]
@@ -77,6 +77,7 @@ def lib() -> C.CDLL:
         L.cudisc_coag_rates_otf.argtypes = [vp, vp, vp, vp, vp]
         L.cudisc_coag_step.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.cudisc_coag_step_host.argtypes = [vp, vp, vp, C.c_double, vp, vp]
+        L.cudisc_coag_step_cached.argtypes = [vp, vp, vp, vp, C.c_double, vp, vp]
         L.cudisc_coag_integrate.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int, dp,
                                             C.POINTER(cudisc_integrate_info), vp]
         L.cudisc_controller_next_dt.argtypes = [C.c_double, C.c_double]
@@ -279,6 +280,14 @@ def _host_ptr(t, name: str, numel: int) -> int:
             or t.numel() != numel:
         raise TypeError(f"{name}: expected a contiguous float64 HOST tensor of {numel} elements")
     return t.data_ptr()
+
+
+def cudisc_coag_step_cached(grid: Grid, bins: Bins, K, rho_dust, dt: float, err_out, stream=None) -> None:
+    """cudisc_coag_step with the kernel read from K [C][2][P] instead of being built."""
+    Cn, N = grid.n_cells, bins.n_bins
+    _check(lib().cudisc_coag_step_cached(grid.handle, bins.handle, _dev_ptr(K, "K", Cn * 2 * bins.n_pairs),
+                                         _dev_ptr(rho_dust, "rho_dust", Cn * N), float(dt),
+                                         _dev_ptr(err_out, "err_out", Cn), _stream(stream)))
 
 
 def cudisc_coag_step_host(grid: Grid, bins: Bins, rho_host, dt: float, err_host, stream=None) -> None:

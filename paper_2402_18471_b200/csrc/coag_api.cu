@@ -752,6 +752,27 @@ int cudisc_coag_step(cudisc_grid g, cudisc_bins b, double *rho_dust, double dt, 
     return rc;
 }
 
+int cudisc_coag_step_cached(cudisc_grid g, cudisc_bins b, const double *K, double *rho_dust, double dt,
+                            double *err_out, cudisc_stream stream)
+{
+    int rc = check_pair(g, b);
+    if (rc) return rc;
+    if (!K || !rho_dust || !err_out) return fail(CUDISC_ERR_INVALID, "NULL array argument");
+    StepArgs sa;
+    memset(&sa, 0, sizeof(sa));
+    sa.Kin = K;
+    sa.rho = rho_dust; sa.rho_out = rho_dust;
+    sa.k_fsal = g->k_fsal; sa.k_out = g->k_fsal;
+    sa.err = err_out;
+    sa.dt = dt; sa.rtol = b->p.rtol; sa.atol_factor = b->p.atol_factor;
+    sa.have_k1 = g->fsal_valid ? 1 : 0;
+    GasArgs ga;
+    memset(&ga, 0, sizeof(ga));
+    rc = run(g, 4, ga, sa, stream);
+    if (rc == CUDISC_OK) g->fsal_valid = true;
+    return rc;
+}
+
 int cudisc_coag_step_host(cudisc_grid g, cudisc_bins b, double *rho_host, double dt,
                           double *err_host, cudisc_stream stream)
 {

@@ -6,12 +6,13 @@
 //   MODE_RATES  : K planes from HBM -> K store, eval   -> drho_dt                     (cudisc_coag_rates)
 //   MODE_OTF    : prologue + pair build -> K store, eval -> drho_dt                   (cudisc_coag_rates_otf)
 //   MODE_STEP   : prologue + pair build -> K store, BS3(2) stages (3 or 4 evals)      (cudisc_coag_step)
+//   MODE_STEPK  : K planes from HBM -> K store, BS3(2) stages                         (cudisc_coag_step_cached)
 // Thread k < N owns bin k: its density, stage values and derivatives live in registers.
 #include "coag_launch.h"
 
 namespace cudisc {
 
-enum { MODE_KERNEL = 0, MODE_RATES = 1, MODE_OTF = 2, MODE_STEP = 3 };
+enum { MODE_KERNEL = 0, MODE_RATES = 1, MODE_OTF = 2, MODE_STEP = 3, MODE_STEPK = 4 };
 
 // ------------------------------------------------------------------------------------------ build
 // K_ij p_coag, K_ij p_frag of every pair of the cell into the K store (or, MODE_KERNEL, to HBM).
@@ -464,7 +465,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
     CellGas nx = {1.0, 1.0, 1.0, 1.0};
     double nvR = 0.0, nvZ = 0.0, nvP = 0.0;
     auto fetch = [&](int cell) {
-        if (MODE == MODE_RATES || cell >= sa.C) return;
+        if (MODE == MODE_RATES || MODE == MODE_STEPK || cell >= sa.C) return;
         nx.T = __ldg(gs.T + cell); nx.rho_g = __ldg(gs.rho_g + cell); nx.Om = __ldg(gs.Omega + cell);
         nx.alpha = gs.alpha ? __ldg(gs.alpha + cell) : gs.alpha_const;
         if (live) {
@@ -483,7 +484,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
         const size_t row = (size_t)cell * N;
 
         // ---------------- K store for this cell
-        if (MODE == MODE_RATES) {
+        if (MODE == MODE_RATES || MODE == MODE_STEPK) {
             // flat, coalesced copy of both planes (8 loads in flight per thread), then the N diagonal
             // entries are halved in place
             const double *k0 = sa.Kin + (size_t)cell * 2 * P, *k1 = k0 + P;
@@ -520,9 +521,9 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
         double y0 = 0.0, k1 = 0.0;
         if (MODE != MODE_KERNEL && live) {
             y0 = sa.rho[row + k];
-            if (MODE == MODE_STEP && sa.have_k1) k1 = sa.k_fsal[row + k];
+            if ((MODE == MODE_STEP || MODE == MODE_STEPK) && sa.have_k1) k1 = sa.k_fsal[row + k];
         }
-        if (MODE != MODE_RATES)
+        if (MODE != MODE_RATES && MODE != MODE_STEPK)
             build_cell<MODE, SLAB>(tb, s, ks, pc, has_vphi,
                                    MODE == MODE_KERNEL ? sa.out + (size_t)cell * 2 * P : nullptr, lane);
         if (MODE == MODE_KERNEL) fetch(cell + gridDim.x);
@@ -552,7 +553,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
                 yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
                 ys = yn;
             }
-            const bool pre = st == 3 && cell + (int)gridDim.x < sa.C;
+            const bool pre = MODE == MODE_STEP && st == 3 && cell + (int)gridDim.x < sa.C;
             const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, tbase, sa_prof, pre, nx, gs.mu,
                                                   gs.sigma_mol, rv);
             if (st == 3) rv_valid = pre;
@@ -611,6 +612,7 @@ static cudaError_t launch_slab(int mode, const LaunchCfg &lc, const DevTables &t
     switch (mode) {
     case MODE_KERNEL: return launch_mode<MODE_KERNEL, SLAB>(lc, tb, gs, sa, st);
     case MODE_RATES: return launch_mode<MODE_RATES, SLAB>(lc, tb, gs, sa, st);
+    case MODE_STEPK: return launch_mode<MODE_STEPK, SLAB>(lc, tb, gs, sa, st);
     case MODE_OTF: return launch_mode<MODE_OTF, SLAB>(lc, tb, gs, sa, st);
     default: return launch_mode<MODE_STEP, SLAB>(lc, tb, gs, sa, st);
     }

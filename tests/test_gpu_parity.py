@@ -245,3 +245,43 @@ def test_full_grid_launch_configuration_sampled_against_oracle():
     m0 = d.rho_dust.sum(axis=1)
     assert np.max(np.abs(rho.sum(axis=1) - m0) / m0) <= TOL_MASS
     assert np.all(np.isfinite(rho)) and np.all(np.isfinite(err))
+
+
+# ------------------------------------------------------------------------------------------ cached-kernel step
+@pytest.mark.parametrize("kind,tau_end,nsteps", [("const", 20.0, 400), ("add", 2.0, 400)])
+def test_cached_step_closed_form_kernels(kind, tau_end, nsteps):
+    """cudisc_coag_step_cached with the closed-form test kernels: the CUDA path against
+    the oracle step by step, and against the analytic zeroth moment M0(t) = N0 / (1 + tau) (constant
+    kernel), N0 exp(-tau) (additive kernel) -- the same pins the oracle itself is held to."""
+    import torch
+    from test_oracle_closed_forms import MBAR, _grid, _initial, _planes
+    N = 120
+    g = _grid(N)
+    Kp = _planes(g, kind, beta=1.0 if kind == "const" else 1.0 / MBAR)
+    rho0 = _initial(g)
+    t_end = 2.0 * tau_end if kind == "const" else tau_end       # tau = K N0 t / 2, resp. beta N0 mbar t
+    dt = t_end / nsteps
+    C = 3
+    pc = cd.Params(v_frag=100.0)
+    bins = cd.Bins(N, g.a_min, g.a_max, g.rho_m, pc)
+    grid = cd.Grid(C, 1, bins)
+    K = torch.from_numpy(np.ascontiguousarray(np.broadcast_to(Kp, (C,) + Kp.shape))).cuda()
+    scale = np.array([1.0, 0.5, 2.0])                            # three cells, different N0
+    rho = torch.from_numpy(rho0[None, :] * scale[:, None]).cuda()
+    err = torch.empty(C, dtype=torch.float64, device="cuda")
+    ref = rho.cpu().numpy().copy()
+    k_ref = None
+    for s in range(nsteps):
+        cd.cudisc_coag_step_cached(grid, bins, K, rho, dt, err)
+        if s < 25:                                               # oracle alongside for the first steps
+            ref, k_ref, e_ref = orc.step_cells_planes(N, g.a_min, g.a_max, g.rho_m, Kp, ref, dt, k1=k_ref)
+            if s in (0, 24):
+                assert_rho_close(rho.cpu().numpy(), ref, TOL_RHO_1 * (s + 1), f"{kind} kernel, step {s + 1}")
+                np.testing.assert_allclose(err.cpu().numpy(), e_ref, rtol=1e-6, atol=1e-12)
+    out = rho.cpu().numpy()
+    m1 = out.sum(axis=1)
+    assert np.max(np.abs(m1 - rho0.sum() * scale) / (rho0.sum() * scale)) <= nsteps * TOL_MASS
+    M0 = (out / g.m_c[None, :]).sum(axis=1)
+    tau = tau_end * scale                                        # tau scales with N0
+    exact = scale / (1.0 + tau) if kind == "const" else scale * np.exp(-tau)
+    np.testing.assert_allclose(M0, exact, rtol=0.06)
