@@ -63,6 +63,10 @@ typedef struct {
     const double *v_R;      /* [C x N] dust radial velocity per size, cm/s                        */
     const double *v_Z;      /* [C x N] dust vertical velocity per size, cm/s                      */
     const double *v_phi;    /* [C x N] or NULL (term left out of Delta v_lam)                     */
+    const double *h_dust;   /* [C x N] dust scale heights, cm, or NULL.  Non-NULL selects the
+                               vertically integrated kernel of PAPER.md:486: K_ij / sqrt(2 pi (h_i^2 +
+                               h_j^2)), rho_dust then holds surface densities and v_Z the settling
+                               velocities at Z = h.  Not together with v_phi (UNSUPPORTED).         */
 } cudisc_gas_state;
 
 /* ---------------------------------------------------------------------------------------------

@@ -203,6 +203,25 @@ def bs32_step(g: MassGrid, K, pf, y, h, k1=None, eta=11.0 / 6.0, chi=1.0, rtol=1
 
 
 # ------------------------------------------------------------------------------------------ batches
+_HD_KEEP = []
+
+
+def _hd(h_dust):
+    """Optional [C x N] dust scale heights (vertically integrated kernel) as a C pointer."""
+    if h_dust is None:
+        return None
+    a = _in(h_dust)
+    _HD_KEEP[:] = [a]
+    return _p(a)
+
+
+def vint_scale(hd, K):
+    """K_ij / sqrt(2 pi (h_i^2 + h_j^2)) of one cell."""
+    K = _in(K).copy(); hd = _in(hd)
+    lib().orc_vint_scale(C.c_int(hd.size), _p(hd), _p(K))
+    return K
+
+
 def _gas_args(T, rho_g, Omega, alpha, vR, vZ, vphi):
     T = _in(T); rho_g = _in(rho_g); Omega = _in(Omega); alpha = _in(alpha); vR = _in(vR); vZ = _in(vZ)
     keep = [T, rho_g, Omega, alpha, vR, vZ]
@@ -212,7 +231,8 @@ def _gas_args(T, rho_g, Omega, alpha, vR, vZ, vphi):
     return keep, [_p(T), _p(rho_g), _p(Omega), _p(alpha), _p(vR), _p(vZ), vp]
 
 
-def kernel_cells(N, a_min, a_max, rho_m, T, rho_g, Omega, alpha, vR, vZ, p: Params, vphi=None) -> np.ndarray:
+def kernel_cells(N, a_min, a_max, rho_m, T, rho_g, Omega, alpha, vR, vZ, p: Params, vphi=None,
+                 h_dust=None) -> np.ndarray:
     """Packed planes [C, 2, P] (plane 0 = K p_coag, plane 1 = K p_frag)."""
     keep, ga = _gas_args(T, rho_g, Omega, alpha, vR, vZ, vphi)
     Cn = keep[0].size
@@ -220,18 +240,18 @@ def kernel_cells(N, a_min, a_max, rho_m, T, rho_g, Omega, alpha, vR, vZ, p: Para
     out = np.empty((Cn, 2, P))
     cp = p.c()
     lib().orc_kernel_cells(C.c_int(Cn), C.c_int(N), C.c_double(a_min), C.c_double(a_max),
-                           C.c_double(rho_m), *ga, C.byref(cp), _p(out))
+                           C.c_double(rho_m), *ga, C.byref(cp), _p(out), _hd(h_dust))
     return out
 
 
-def rates_cells(N, a_min, a_max, rho_m, T, rho_g, Omega, alpha, vR, vZ, p: Params, rho, vphi=None):
+def rates_cells(N, a_min, a_max, rho_m, T, rho_g, Omega, alpha, vR, vZ, p: Params, rho, vphi=None, h_dust=None):
     keep, ga = _gas_args(T, rho_g, Omega, alpha, vR, vZ, vphi)
     rho = _in(rho)
     Cn = keep[0].size
     d = np.empty((Cn, N)); g = np.empty((Cn, N)); l = np.empty((Cn, N))
     cp = p.c()
     lib().orc_rates_cells(C.c_int(Cn), C.c_int(N), C.c_double(a_min), C.c_double(a_max),
-                          C.c_double(rho_m), *ga, C.byref(cp), _p(rho), _p(d), _p(g), _p(l))
+                          C.c_double(rho_m), *ga, C.byref(cp), _p(rho), _p(d), _p(g), _p(l), _hd(h_dust))
     return d, g, l
 
 
@@ -248,7 +268,7 @@ def rates_cells_planes(N, a_min, a_max, rho_m, Kp, rho, eta=11.0 / 6.0, chi=1.0)
 
 
 def step_cells(N, a_min, a_max, rho_m, T, rho_g, Omega, alpha, vR, vZ, p: Params, rho, dt, k1=None,
-               vphi=None):
+               vphi=None, h_dust=None):
     """One BS3(2) step of every cell.  Returns rho_new [C,N], k4 [C,N], err [C]."""
     keep, ga = _gas_args(T, rho_g, Omega, alpha, vR, vZ, vphi)
     rho = _in(rho).copy()
@@ -259,7 +279,7 @@ def step_cells(N, a_min, a_max, rho_m, T, rho_g, Omega, alpha, vR, vZ, p: Params
     cp = p.c()
     lib().orc_step_cells(C.c_int(Cn), C.c_int(N), C.c_double(a_min), C.c_double(a_max),
                          C.c_double(rho_m), *ga, C.byref(cp), _p(rho), _p(k), C.c_int(1 if have else 0),
-                         C.c_double(dt), _p(err))
+                         C.c_double(dt), _p(err), _hd(h_dust))
     return rho, k, err
 
 

@@ -22,6 +22,7 @@
  *   orc_frag_redistribute .... pinned (telescoping sum = 1; brute force against Eq. 67 directly)
  *   orc_bs32_step ............ pinned (order of convergence 3, exact on cubic-in-t test ODE via
  *                              the generic-rhs twin in the tests; conservation 1e-13)
+ *   orc_vint_scale ........... pinned (quadrature of the product of two Gaussian vertical profiles)
  *   orc_cell_kernel .......... Brownian/laminar parts + regime limits of the turbulent part pinned;
  *                              PARITY UNPINNED for: sigma_ij = pi (a_i+a_j)^2 (R3), the Ormel &
  *                              Cuzzi formulas as recalled (R4, limits pinned only), nu_mol (R6),
@@ -166,6 +167,18 @@ void orc_cell_kernel(int N, const double *a_c, const double *m_c, double rho_m,
         }
     }
     free(St); free(Ss);
+}
+
+/* Vertically integrated kernel: "constructed by dividing the coagulation kernel (Eqn. 56)
+ * by sqrt(2 pi (h_i^2 + h_j^2)), where h_i & h_j are the scale heights of the dust grains, assuming a
+ * Gaussian vertical density profile".  hd[N]: dust scale heights (an input, like the velocities).
+ * K: full N x N, scaled in place; p_frag is a function of dv only and stays.
+ * Pinned (tests/test_oracle_pins.py) by numerical quadrature of the product of two Gaussians. */
+void orc_vint_scale(int N, const double *hd, double *K)
+{
+    for (int i = 0; i < N; ++i)
+        for (int j = 0; j < N; ++j)
+            K[i * N + j] /= sqrt(2.0 * ORC_PI * (hd[i] * hd[i] + hd[j] * hd[j]));
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -449,7 +462,7 @@ static void unpack_planes(int N, const double *Kp, double *Kc, double *Kf)
 void orc_kernel_cells(int C, int N, double a_min, double a_max, double rho_m,
                       const double *T, const double *rho_g, const double *Omega, const double *alpha,
                       const double *vR, const double *vZ, const double *vphi,
-                      const orc_params *p, double *K_out)
+                      const orc_params *p, double *K_out, const double *hd)
 {
     size_t P = (size_t)N * (N + 1) / 2;
     double *m_e, *a_c, *m_c;
@@ -463,6 +476,7 @@ void orc_kernel_cells(int C, int N, double a_min, double a_max, double rho_m,
             orc_cell_kernel(N, a_c, m_c, rho_m, T[c], rho_g[c], Omega[c], alpha[c],
                             vR + (size_t)c * N, vZ + (size_t)c * N, vphi ? vphi + (size_t)c * N : NULL,
                             p, K, pf, NULL, NULL);
+            if (hd) orc_vint_scale(N, hd + (size_t)c * N, K);
             to_products(N, K, pf);
             double *o0 = K_out + (size_t)c * 2 * P, *o1 = o0 + P;
             for (int i = 0; i < N; ++i)
@@ -505,7 +519,8 @@ void orc_rates_cells_planes(int C, int N, double a_min, double a_max, double rho
 void orc_rates_cells(int C, int N, double a_min, double a_max, double rho_m,
                      const double *T, const double *rho_g, const double *Omega, const double *alpha,
                      const double *vR, const double *vZ, const double *vphi,
-                     const orc_params *p, const double *rho, double *drho, double *gain, double *loss)
+                     const orc_params *p, const double *rho, double *drho, double *gain, double *loss,
+                     const double *hd)
 {
     double *m_e, *a_c, *m_c;
     double *a_e = grid_alloc(N, a_min, a_max, rho_m, &m_e, &a_c, &m_c);
@@ -518,6 +533,7 @@ void orc_rates_cells(int C, int N, double a_min, double a_max, double rho_m,
             orc_cell_kernel(N, a_c, m_c, rho_m, T[c], rho_g[c], Omega[c], alpha[c],
                             vR + (size_t)c * N, vZ + (size_t)c * N, vphi ? vphi + (size_t)c * N : NULL,
                             p, K, pf, NULL, NULL);
+            if (hd) orc_vint_scale(N, hd + (size_t)c * N, K);
             to_products(N, K, pf);
             orc_rates_flux_cf(N, m_c, m_e, K, pf, rho + (size_t)c * N, p->eta, p->chi_im,
                               drho + (size_t)c * N, gain ? gain + (size_t)c * N : NULL,
@@ -533,7 +549,8 @@ void orc_rates_cells(int C, int N, double a_min, double a_max, double rho_m,
 void orc_step_cells(int C, int N, double a_min, double a_max, double rho_m,
                     const double *T, const double *rho_g, const double *Omega, const double *alpha,
                     const double *vR, const double *vZ, const double *vphi,
-                    const orc_params *p, double *rho, double *k1, int have_k1, double dt, double *err)
+                    const orc_params *p, double *rho, double *k1, int have_k1, double dt, double *err,
+                    const double *hd)
 {
     double *m_e, *a_c, *m_c;
     double *a_e = grid_alloc(N, a_min, a_max, rho_m, &m_e, &a_c, &m_c);
@@ -546,6 +563,7 @@ void orc_step_cells(int C, int N, double a_min, double a_max, double rho_m,
             orc_cell_kernel(N, a_c, m_c, rho_m, T[c], rho_g[c], Omega[c], alpha[c],
                             vR + (size_t)c * N, vZ + (size_t)c * N, vphi ? vphi + (size_t)c * N : NULL,
                             p, K, pf, NULL, NULL);
+            if (hd) orc_vint_scale(N, hd + (size_t)c * N, K);
             to_products(N, K, pf);
             err[c] = orc_bs32_step(N, m_c, m_e, K, pf, p->eta, p->chi_im, p->rtol, p->atol_factor,
                                    rho + (size_t)c * N, k1 + (size_t)c * N, have_k1, dt);

@@ -33,7 +33,7 @@ class cudisc_params(C.Structure):
 
 class cudisc_gas_state(C.Structure):
     _fields_ = [("T", C.c_void_p), ("rho_gas", C.c_void_p), ("Omega", C.c_void_p), ("alpha", C.c_void_p),
-                ("v_R", C.c_void_p), ("v_Z", C.c_void_p), ("v_phi", C.c_void_p)]
+                ("v_R", C.c_void_p), ("v_Z", C.c_void_p), ("v_phi", C.c_void_p), ("h_dust", C.c_void_p)]
 
 
 class cudisc_integrate_info(C.Structure):
@@ -212,17 +212,18 @@ class Grid:
     def handle(self):
         return self._h
 
-    def _gas_struct(self, T, rho_gas, Omega, v_R, v_Z, alpha=None, v_phi=None):
+    def _gas_struct(self, T, rho_gas, Omega, v_R, v_Z, alpha=None, v_phi=None, h_dust=None):
         Cn, N = self.n_cells, self.bins.n_bins
         gs = cudisc_gas_state(
             _dev_ptr(T, "T", Cn), _dev_ptr(rho_gas, "rho_gas", Cn), _dev_ptr(Omega, "Omega", Cn),
             _dev_ptr(alpha, "alpha", Cn) if alpha is not None else None,
             _dev_ptr(v_R, "v_R", Cn * N), _dev_ptr(v_Z, "v_Z", Cn * N),
-            _dev_ptr(v_phi, "v_phi", Cn * N) if v_phi is not None else None)
-        return gs, (T, rho_gas, Omega, alpha, v_R, v_Z, v_phi)
+            _dev_ptr(v_phi, "v_phi", Cn * N) if v_phi is not None else None,
+            _dev_ptr(h_dust, "h_dust", Cn * N) if h_dust is not None else None)
+        return gs, (T, rho_gas, Omega, alpha, v_R, v_Z, v_phi, h_dust)
 
-    def bind_gas(self, T, rho_gas, Omega, v_R, v_Z, alpha=None, v_phi=None):
-        gs, keep = self._gas_struct(T, rho_gas, Omega, v_R, v_Z, alpha, v_phi)
+    def bind_gas(self, T, rho_gas, Omega, v_R, v_Z, alpha=None, v_phi=None, h_dust=None):
+        gs, keep = self._gas_struct(T, rho_gas, Omega, v_R, v_Z, alpha, v_phi, h_dust)
         _check(lib().cudisc_grid_bind_gas(self._h, C.byref(gs)))
         self._gas_keep = keep      # the library keeps the pointers, not the arrays
 

@@ -350,7 +350,7 @@ GasArgs gas_args(const cudisc_gas_state &gs, const cudisc_params &p)
 {
     GasArgs g;
     g.T = gs.T; g.rho_g = gs.rho_gas; g.Omega = gs.Omega; g.alpha = gs.alpha;
-    g.vR = gs.v_R; g.vZ = gs.v_Z; g.vphi = gs.v_phi;
+    g.vR = gs.v_R; g.vZ = gs.v_Z; g.vphi = gs.v_phi; g.hd = gs.h_dust;
     g.alpha_const = p.alpha; g.mu = p.mu; g.v_frag = p.v_frag; g.sigma_mol = p.sigma_mol;
     return g;
 }
@@ -360,6 +360,8 @@ int check_gas(const cudisc_gas_state *gs)
     if (!gs) return fail(CUDISC_ERR_INVALID, "gas_state is NULL");
     if (!gs->T || !gs->rho_gas || !gs->Omega || !gs->v_R || !gs->v_Z)
         return fail(CUDISC_ERR_INVALID, "gas_state: T, rho_gas, Omega, v_R and v_Z must be non-NULL");
+    if (gs->v_phi && gs->h_dust)
+        return fail(CUDISC_ERR_UNSUPPORTED, "gas_state: v_phi and h_dust cannot both be given");
     return CUDISC_OK;
 }
 

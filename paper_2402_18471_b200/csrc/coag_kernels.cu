@@ -385,7 +385,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     return d;
 }
 
-template <int NT, int MODE, bool SLAB>
+template <int NT, int MODE, bool SLAB, bool VINT>
 __global__ void __launch_bounds__(NT, 1)
 coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
 {
@@ -400,6 +400,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
                          tb.nBuildItems, tb.nEvalItems, tb.bandD);
     PairConst pc;
     const bool has_vphi = gs.vphi != nullptr;
+    constexpr bool has_h = VINT;        // vertically integrated kernel: its own instantiation
     pc.c15vf2 = 1.5 * gs.v_frag * gs.v_frag;
     pc.Vg2 = 0.0;
 
@@ -472,6 +473,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
             const size_t g = (size_t)cell * N + k;
             nvR = __ldg(gs.vR + g); nvZ = __ldg(gs.vZ + g);
             if (has_vphi) nvP = __ldg(gs.vphi + g);
+            if (has_h) nvP = __ldg(gs.hd + g);
         }
     };
     fetch(blockIdx.x);
@@ -510,7 +512,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
             }
         } else {
             if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, s, k);
-            prologue_store(tb, rv, nvR, nvZ, nvP, has_vphi, s, k);
+            prologue_store(tb, rv, nvR, nvZ, nvP, has_vphi, has_h, s, k);
             // V_g^2 through shared memory: only the bin-owning warps hold the pre-computed values
             if (tid == 0) { s.CTR[0] = NT / 32; s.RED[95] = rv.Vg2; }
             __syncthreads();
@@ -528,6 +530,25 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
                                    MODE == MODE_KERNEL ? sa.out + (size_t)cell * 2 * P : nullptr, lane);
         if (MODE == MODE_KERNEL) fetch(cell + gridDim.x);
         __syncthreads();
+        // vertically integrated kernel: every K_ij / sqrt(2 pi (h_i^2 + h_j^2)); p_frag is
+        // unchanged, so both planes take the factor.  A separate sweep keeps the pair loops as they are.
+        if (MODE != MODE_RATES && MODE != MODE_STEPK && has_h) {
+            for (int i = tid >> 5; i < N; i += NT / 32) {
+                const double hi2 = s.V5[i];
+                const int base = tri(i);
+                for (int j = lane; j <= i; j += 32) {
+                    const double f = 1.0 / sqrt((2.0 * kPiD) * (hi2 + s.V5[j]));
+                    if (MODE == MODE_KERNEL) {
+                        double *o = sa.out + (size_t)cell * 2 * P;
+                        o[base + j] *= f; o[P + base + j] *= f;
+                    } else {
+                        const double2 v = ks.ld(base + j);
+                        ks.st(base + j, make_double2(v.x * f, v.y * f));
+                    }
+                }
+            }
+            __syncthreads();
+        }
         PROF_ADD(1, tc0);
         if (MODE == MODE_KERNEL) continue;
 
@@ -588,12 +609,12 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
 }
 
 // ------------------------------------------------------------------------------------------ launch
-template <int MODE, bool SLAB>
-static cudaError_t launch_mode(const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
+template <int MODE, bool SLAB, bool VINT>
+static cudaError_t launch_vint(const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
                                const StepArgs &sa, cudaStream_t st)
 {
     constexpr int NT = kThreads;
-    auto fn = coag_cells_kernel<NT, MODE, SLAB>;
+    auto fn = coag_cells_kernel<NT, MODE, SLAB, VINT>;
     static bool attr_done = false;          // per process and per instantiation; same value every time
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -603,6 +624,15 @@ static cudaError_t launch_mode(const LaunchCfg &lc, const DevTables &tb, const G
     }
     fn<<<lc.grid, NT, lc.smem_bytes, st>>>(tb, gs, sa);
     return cudaGetLastError();
+}
+
+template <int MODE, bool SLAB>
+static cudaError_t launch_mode(const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
+                               const StepArgs &sa, cudaStream_t st)
+{
+    // the modes that read K from HBM never see a gas state
+    if (MODE != MODE_RATES && MODE != MODE_STEPK && gs.hd) return launch_vint<MODE, SLAB, true>(lc, tb, gs, sa, st);
+    return launch_vint<MODE, SLAB, false>(lc, tb, gs, sa, st);
 }
 
 template <bool SLAB>
@@ -628,7 +658,7 @@ cudaError_t launch_cells(int mode, const LaunchCfg &lc, const DevTables &tb, con
 
 int cells_occupancy(int smem_bytes, int smem_optin)
 {
-    auto fn = coag_cells_kernel<kThreads, MODE_STEP, true>;
+    auto fn = coag_cells_kernel<kThreads, MODE_STEP, true, false>;
     if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
         return 0;
     int n = 0;

@@ -285,3 +285,37 @@ def test_cached_step_closed_form_kernels(kind, tau_end, nsteps):
     tau = tau_end * scale                                        # tau scales with N0
     exact = scale / (1.0 + tau) if kind == "const" else scale * np.exp(-tau)
     np.testing.assert_allclose(M0, exact, rtol=0.06)
+
+
+# ------------------------------------------------------------------------------------------ vertically integrated kernel
+def test_vertically_integrated_kernel_matches_oracle():
+    """h_dust given -> K / sqrt(2 pi (h_i^2 + h_j^2)); kernel, rates and
+    steps against the oracle on config 1 with seeded scale heights; v_phi together with h_dust is refused."""
+    import torch
+    cfg, d = _disc(1)
+    po, pc = params_pair(cfg)
+    rng = np.random.default_rng(9)
+    H = np.sqrt(synth_disc.K_B * d.T / (cfg.mu * synth_disc.M_H)) / d.Omega
+    h = H[:, None] * np.exp(-rng.uniform(0.0, 3.0, size=d.v_R.shape))       # h_i <= H, seeded
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    g = GpuDisc(d, pc)
+    gas = dict(g.gas); gas["h_dust"] = t(h)
+    g.grid.bind_gas(**gas)
+    K = torch.empty((d.n_cells, 2, g.P), dtype=torch.float64, device="cuda")
+    cd.cudisc_coag_kernel(g.grid, g.bins, gas, pc, K)
+    Kref = orc.kernel_cells(*oracle_args(d), po, h_dust=h)
+    Ktot = Kref[:, 0] + Kref[:, 1]
+    assert np.all(np.abs(K.cpu().numpy() - Kref) <= TOL_K * Ktot[:, None, :])
+    K0 = orc.kernel_cells(*oracle_args(d), po)
+    assert np.max(np.abs(Kref / np.where(K0 > 0, K0, 1.0) - 1.0)) > 0.5      # the factor really entered
+    dt = 1e-3 * dt_of(1) * float(np.median(np.sqrt(2.0 * np.pi * 2.0) * h))  # rates scale with 1/h
+    rho = g.rho.clone()
+    rho_ref, k_ref = d.rho_dust.copy(), None
+    for s in range(3):
+        rho_ref, k_ref, err_ref = orc.step_cells(*oracle_args(d), po, rho_ref, dt, k1=k_ref, h_dust=h)
+        err = g.step(rho, dt)
+    assert_rho_close(rho.cpu().numpy(), rho_ref, 3 * TOL_RHO_1, "vertically integrated, 3 steps")
+    np.testing.assert_allclose(err.cpu().numpy(), err_ref, rtol=1e-6, atol=1e-12)
+    with pytest.raises(cd.CudiscError):
+        gas2 = dict(gas); gas2["v_phi"] = t(np.zeros_like(h))
+        g.grid.bind_gas(**gas2)

@@ -227,3 +227,36 @@ def test_lbin_is_smallest_l_with_upper_edge_above():
         assert l == min(k for k in range(g.N) if g.m_e[k + 1] > m)
     for k in range(g.N):
         assert orc.lbin(g, g.m_c[k]) == k         # a grid mass belongs to its own bin
+
+
+def test_vertically_integrated_kernel_is_the_overlap_of_two_gaussians():
+    """the kernel divided by sqrt(2 pi (h_i^2 + h_j^2)) 'assuming a Gaussian vertical
+    density profile': that factor is the vertical integral of the product of two unit-surface-density
+    Gaussians, checked here by quadrature (not by retyping the formula)."""
+    from scipy.integrate import quad
+    hd = np.array([0.3, 1.0, 2.5, 7.0])
+    K = np.arange(1.0, 17.0).reshape(4, 4)
+    K = K + K.T
+    Ks = orc.vint_scale(hd, K)
+    gauss = lambda z, h: np.exp(-0.5 * (z / h) ** 2) / (np.sqrt(2.0 * np.pi) * h)
+    for i in range(4):
+        for j in range(4):
+            w = min(hd[i], hd[j])
+            overlap, _ = quad(lambda z: gauss(z, hd[i]) * gauss(z, hd[j]), -40.0 * w, 40.0 * w,
+                              epsabs=0.0, epsrel=1e-12, limit=400)
+            assert Ks[i, j] == pytest.approx(K[i, j] * overlap, rel=1e-10)
+    # the batch driver applies it to K only: p_frag (a function of dv) is unchanged
+    N, C = 12, 3
+    rng = np.random.default_rng(2)
+    a = dict(T=np.full(C, 80.0), rho_g=np.full(C, 1e-12), Omega=np.full(C, 2e-9), alpha=np.full(C, 1e-3),
+             vR=rng.normal(scale=10.0, size=(C, N)), vZ=rng.normal(scale=10.0, size=(C, N)))
+    h = 1e12 * np.exp(rng.normal(size=(C, N)))
+    p = orc.Params()
+    K0 = orc.kernel_cells(N, 1e-4, 1.0, 1.67, a["T"], a["rho_g"], a["Omega"], a["alpha"], a["vR"], a["vZ"], p)
+    K1 = orc.kernel_cells(N, 1e-4, 1.0, 1.67, a["T"], a["rho_g"], a["Omega"], a["alpha"], a["vR"], a["vZ"], p,
+                          h_dust=h)
+    iu = np.tril_indices(N)
+    for c in range(C):
+        f = 1.0 / np.sqrt(2.0 * np.pi * (h[c][:, None] ** 2 + h[c][None, :] ** 2))
+        np.testing.assert_allclose(K1[c, 0], K0[c, 0] * f[iu], rtol=1e-14)
+        np.testing.assert_allclose(K1[c, 1], K0[c, 1] * f[iu], rtol=1e-14)
