@@ -418,7 +418,7 @@ double orc_bs32_step(int N, const double *m_c, const double *m_e, const double *
     for (int k = 0; k < N; ++k) {
         double e = h * ((-5.0 / 72.0) * k1[k] + (1.0 / 12.0) * k2[k] + (1.0 / 9.0) * k3[k] - (1.0 / 8.0) * k4[k]);
         double sc = atol + rtol * fmax(fabs(y[k]), fabs(yn[k]));
-        double r = fabs(e) / sc;
+        double r = (e == 0.0) ? 0.0 : fabs(e) / sc;   /* R10: e_k = 0 counts 0 (an empty cell has sc = 0: no 0/0) */
         if (r > E || r != r) E = r;
     }
     for (int k = 0; k < N; ++k) { y[k] = yn[k]; k1[k] = k4[k]; }

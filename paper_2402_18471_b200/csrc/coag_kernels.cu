@@ -592,7 +592,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
         if (live) {
             const double e = h * ((-5.0 / 72.0) * k1 + (1.0 / 12.0) * k2 + (1.0 / 9.0) * k3 - (1.0 / 8.0) * k4);
             const double sc = atol + sa.rtol * fmax(fabs(y0), fabs(yn));
-            emax = fabs(e) / sc;
+            emax = (e == 0.0) ? 0.0 : fabs(e) / sc;      // R10: a bin with no error estimate (empty cell: 0/0) counts 0
             sa.rho_out[row + k] = yn;
             sa.k_out[row + k] = k4;
         }

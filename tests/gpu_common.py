@@ -125,3 +125,33 @@ def assert_rates_close(d_gpu, d_ref, gain, loss, tol=TOL_RATE, what=""):
                              f"gain+loss {scale[w]:.3e}")
     nz = scale > RATE_ABS_FLOOR / tol
     return float((diff[nz] / scale[nz]).max()) if nz.any() else 0.0
+
+
+def assert_planes_strict(K_gpu, K_ref, what=""):
+    """SURVEY 8(c) "rel. 1e-12 per entry", applied to each plane on its own: 1e-12 where p_coag and p_frag
+    both exceed 1e-2, 1e-11 where they exceed 1e-3.  Eq. 55's K p_coag = K - K p_frag carries an ABSOLUTE
+    error of a few u K_ij on either side, i.e. a relative one of a few u / p: the
+    per-entry bar is only meaningful where p is not small, and elsewhere the bar is TOL_K * K_ij.
+    K_*: [2, P].  Returns the number of entries checked at 1e-12."""
+    Kt = K_ref[0] + K_ref[1]
+    n = 0
+    for pmin, tol in ((1e-2, TOL_K), (1e-3, 10 * TOL_K)):
+        ok = (K_ref[0] > pmin * Kt) & (K_ref[1] > pmin * Kt)
+        for plane in (0, 1):
+            rel = np.abs(K_gpu[plane] - K_ref[plane])[ok] / K_ref[plane][ok]
+            assert rel.size == 0 or rel.max() <= tol, \
+                f"{what}: plane {plane} strict rel diff {rel.max():.3e} (p > {pmin})"
+        n = n or int(ok.sum())
+    return n
+
+
+def strict_rate_scale(d, po, cfg):
+    """The oracle's OWN gain + loss magnitudes (real p_coag, p_frag) and the bins where they are the valid
+    scale of the on-the-fly rate comparison: those whose magnitude is at least 1e-3 of the split-free one
+    (the pairs feeding them have effective probabilities above 1e-3, so Eq. 55's absolute error u K_ij is
+    at most 1e3 u of the true terms)."""
+    _, gain, loss = orc.rates_cells(*oracle_args(d), po, d.rho_dust)
+    gfree, lfree = split_free_magnitudes(d, po, cfg)
+    scale = gain + loss
+    ok = (scale >= 1e-3 * (gfree + lfree)) & (scale > 0)
+    return scale, ok
