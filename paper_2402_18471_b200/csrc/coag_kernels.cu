@@ -12,7 +12,6 @@
 
 namespace cudisc {
 
-enum { MODE_KERNEL = 0, MODE_RATES = 1, MODE_OTF = 2, MODE_STEP = 3, MODE_STEPK = 4 };
 
 // ------------------------------------------------------------------------------------------ build
 // K_ij p_coag, K_ij p_frag of every pair of the cell into the K store (or, MODE_KERNEL, to HBM).
@@ -124,7 +123,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
 
     // per-bin values of the NEXT cell (inputs were fetched an evaluation ago): the bin-owning warps
     // compute them here, in registers, while the other warps start on the items
-    if (pre && 32 * warp < N) rv = prologue_compute(tb, nx, mu, sigma_mol, s, k);
+    if (pre && 32 * warp < N) rv = prologue_compute(tb, nx, mu, sigma_mol, live ? s.BINC[BC_RM * Np + k] : 0.0, k);
 
     // ---- phase A: band gathers from tensor memory (tasks fixed per warp: a warp only reaches the
     //      tensor-memory lanes of its quarter), then row sums, column sums (and, without
@@ -511,7 +510,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
                 ks.st(p, make_double2(0.5 * v.x, 0.5 * v.y));
             }
         } else {
-            if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, s, k);
+            if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, live ? s.BINC[BC_RM * tb.Np + k] : 0.0, k);
             prologue_store(tb, rv, nvR, nvZ, nvP, has_vphi, has_h, s, k);
             // V_g^2 through shared memory: only the bin-owning warps hold the pre-computed values
             if (tid == 0) { s.CTR[0] = NT / 32; s.RED[95] = rv.Vg2; }
@@ -615,12 +614,14 @@ static cudaError_t launch_vint(const LaunchCfg &lc, const DevTables &tb, const G
 {
     constexpr int NT = kThreads;
     auto fn = coag_cells_kernel<NT, MODE, SLAB, VINT>;
-    static bool attr_done = false;          // per process and per instantiation; same value every time
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             lc.smem_optin);
+    static bool attr_done[64] = {false};    // the attribute is per device (and per instantiation)
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !attr_done[dev]) {
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, lc.smem_optin);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        if (dev >= 0 && dev < 64) attr_done[dev] = true;
     }
     fn<<<lc.grid, NT, lc.smem_bytes, st>>>(tb, gs, sa);
     return cudaGetLastError();
