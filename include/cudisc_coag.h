@@ -120,8 +120,19 @@ int cudisc_bins_expand_outcomes(cudisc_bins b, long long *n_entries, int *target
  *   out[4] band indices out of range of what they address, or band entries lost
  *   out[5] band gather tasks: target groups without exactly one covering set of tasks
  *   out[6] number of items (build + eval);  out[7] shared-memory bytes needed besides the K store
- * out[0..5] are 0 for a correct schedule.  out: HOST [8]. */
+ * out[0..5] are 0 for a correct schedule.  out: HOST [8].  When the grid takes the tensor-memory kernel
+ * (cudisc_bins_fast_path) its static per-warp task lists are checked as well and counted in the same
+ * slots: pairs built once, bulk (row, column) and (i >= j) summed once, partial-sum parts written once,
+ * tensor-memory columns written by the build exactly where the column tasks of the same quarter read them
+ * and disjoint from the tables, band entries complete, at most two band halves per warp. */
 int cudisc_bins_schedule_check(cudisc_bins b, long long *out);
+
+/* Whether this mass grid takes the tensor-memory kernel for cudisc_coag_step / cudisc_coag_rates_otf
+ * (second copy of the cell's kernel in the SM's tensor memory, static per-warp
+ * schedule; needs 64 <= n_bins, the band tables and the row copy to fit: up to ~155 bins at 227 KB of
+ * shared memory), the dynamic shared memory it needs and the 32-bit tensor-memory columns (of 4 x 512)
+ * its tables and column copy occupy.  Otherwise the general kernel runs (any n_bins <= 256).  Host only. */
+int cudisc_bins_fast_path(cudisc_bins b, int *on, long long *smem_bytes, int *tmem_cols_used);
 
 /* Cell grid of n_r x n_z cells using mass grid b.  Allocates on the current CUDA device: the
  * FSAL buffer [C x N], and the kernel scratch.  The handle remembers b. */

@@ -43,7 +43,7 @@ class cudisc_integrate_info(C.Structure):
 
 EXPORTS = [
     "cudisc_bins_create", "cudisc_bins_create_general", "cudisc_bins_destroy", "cudisc_bins_query",
-    "cudisc_bins_expand_outcomes", "cudisc_bins_schedule_check", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
+    "cudisc_bins_expand_outcomes", "cudisc_bins_schedule_check", "cudisc_bins_fast_path", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
     "cudisc_grid_destroy", "cudisc_coag_kernel", "cudisc_coag_rates", "cudisc_coag_rates_otf",
     "cudisc_coag_step", "cudisc_coag_step_cached", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_controller_next_dt",
     "cudisc_microbench_dfma",
@@ -68,6 +68,7 @@ def lib() -> C.CDLL:
         L.cudisc_bins_query.argtypes = [vp, ip, dp, dp, dp, ip, ip]
         L.cudisc_bins_expand_outcomes.argtypes = [vp, C.POINTER(C.c_longlong), ip, ip, ip, ip, dp, dp, dp]
         L.cudisc_bins_schedule_check.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.cudisc_bins_fast_path.argtypes = [vp, ip, C.POINTER(C.c_longlong), ip]
         L.cudisc_grid_create.argtypes = [C.c_int, C.c_int, vp, C.POINTER(vp)]
         L.cudisc_grid_bind_gas.argtypes = [vp, C.POINTER(cudisc_gas_state)]
         L.cudisc_grid_reset_fsal.argtypes = [vp]
@@ -184,6 +185,12 @@ class Bins:
         out = (C.c_longlong * 8)()
         _check(lib().cudisc_bins_schedule_check(self._h, out))
         return [int(v) for v in out]
+
+    def fast_path(self):
+        """(on, shared-memory bytes, tensor-memory columns) of the tensor-memory kernel for this grid."""
+        on = C.c_int(); sm = C.c_longlong(); tm = C.c_int()
+        _check(lib().cudisc_bins_fast_path(self._h, C.byref(on), C.byref(sm), C.byref(tm)))
+        return bool(on.value), int(sm.value), int(tm.value)
 
     def close(self):
         if self._h:

@@ -536,8 +536,8 @@ void build_fast_schedule(const HostTables &t, const Schedule &S, FastSchedule &F
     deal(bjobs, F.buildTasks, f.bw, nullptr);
     deal(ejobs, F.evalTasks, f.ew, pre);
 
-    F.smemDoubles = 2 * (size_t)d.P + fast_misc_doubles(d.Np, (int)(F.buildTasks.size() + F.evalTasks.size()))
-                    + fast_union_doubles(d.Np, f.nRowParts, f.nColParts, d.bandD);
+    fast_layout(f, d.P, d.Np, d.bandD);
+    F.smemDoubles = (size_t)f.off[FO_END];
     f.on = 1;
     F.f = f;
 }
@@ -834,10 +834,139 @@ int cudisc_bins_schedule_check(cudisc_bins b, long long *out)
             if (ntask < 1 || ntask > 2 || ent != Lg) ++bad[5];
         }
     }
+    // ---- the static schedule of the tensor-memory kernel, when this grid takes it (coag_fast.h): same
+    //      counters.  Tasks are decoded with ftask_unpack, the function the device uses.
+    FastSchedule F;
+    build_fast_schedule(t, S, F);
+    if (F.f.on) {
+        const FastTables &f = F.f;
+        const int nWarps = kThreads / 32;
+        std::vector<int> fbuilt((size_t)N * N, 0), frow((size_t)N * N, 0), fcol((size_t)N * N, 0);
+        // tensor-memory map: (quarter, column) -> row-slice id c * 4096 + i written by the build, read by COLT
+        std::vector<int> tmap(4 * kTmemCols, -1), tread(4 * kTmemCols, 0);
+        auto claim = [&](int q, int col, int n, int id) {        // band / per-bin constant regions
+            for (int u = col; u < col + n; ++u) {
+                if (u < 0 || u >= kTmemCols || tmap[q * kTmemCols + u] != -1) { ++bad[3]; continue; }
+                tmap[q * kTmemCols + u] = id;
+            }
+        };
+        for (int q = 0; q < 4; ++q) claim(q, 0, fast_binc_cols(f.nwBins), -2);
+        for (int gh = 0; gh < 2 * f.nwBins; ++gh) claim(f.bgWarp[gh] & 3, f.bgCol[gh], 3 * f.bgLen[gh], -3);
+        for (int g = 0; g < f.nwBins; ++g) claim((f.nwBins + g) & 3, f.sgCol[g], 3 * f.sgLen[g], -4);
+        for (int w = 0; w < nWarps; ++w)
+            for (int it = f.bw[w]; it < f.bw[w + 1]; ++it) {
+                const FTask k = ftask_unpack(F.buildTasks[it]);
+                if (k.kind == FB_ROWS) {
+                    for (int i = k.a; i < k.b; ++i)
+                        for (int lane = 0; lane < 32; ++lane) {
+                            const int j = 32 * k.blk + lane;
+                            if (j >= N) continue;
+                            if (i >= N || j >= i) { ++bad[0]; continue; }
+                            fbuilt[(size_t)i * N + j]++;
+                        }
+                    if (k.tcol != kNoTmem)
+                        for (int i = k.a; i < k.a + ((k.b - k.a + 1) & ~1); ++i) claim(w & 3, k.tcol + 4 * (i - k.a), 4, k.blk * 4096 + i);
+                } else {
+                    for (int tt = k.a; tt < k.b; ++tt) {
+                        int r = (int)((std::sqrt(8.0 * tt + 1.0) - 1.0) * 0.5);
+                        while (tri_h(r + 1) <= tt) ++r;
+                        while (tri_h(r) > tt) --r;
+                        const int i = 32 * k.blk + r, j = 32 * k.blk + (tt - tri_h(r));
+                        if (i >= N || j > i) { ++bad[0]; continue; }
+                        fbuilt[(size_t)i * N + j]++;
+                    }
+                }
+            }
+        std::vector<int> rpart(std::max(1, f.nRowParts), 0), cpart(std::max(1, f.nColParts), 0);
+        int nWtask = 0;
+        for (int w = 0; w < nWarps; ++w)
+            for (int it = f.ew[w]; it < f.ew[w + 1]; ++it) {
+                const FTask k = ftask_unpack(F.evalTasks[it]);
+                if (k.kind == FE_RECT || k.kind == FE_RAG) {
+                    if (k.slot < f.rpBase[k.blk] || k.slot >= f.rpBase[k.blk] + f.rpCnt[k.blk] || rpart[k.slot]++) ++bad[3];
+                    if (k.kind == FE_RECT && ((k.a | k.b) & 1)) ++bad[1];
+                    for (int i = 32 * k.blk; i < std::min(N, 32 * k.blk + 32); ++i)
+                        for (int j = k.a; j < k.b; ++j) {
+                            if (k.kind == FE_RECT && j >= t.n_bulk[i]) ++bad[1];      // the rectangle must be bulk
+                            if (j < t.n_bulk[i]) frow[(size_t)i * N + j]++;
+                        }
+                } else if (k.kind == FE_COLT || k.kind == FE_COLS) {
+                    if (k.slot < f.cpBase[k.blk] || k.slot >= f.cpBase[k.blk] + f.cpCnt[k.blk] || cpart[k.slot]++) ++bad[3];
+                    for (int i = k.a; i < k.b; ++i)
+                        for (int j = 32 * k.blk; j < std::min(N, 32 * k.blk + 32); ++j)
+                            if (i >= j) fcol[(size_t)i * N + j]++;
+                    if (k.kind == FE_COLT) {
+                        if (k.a < 32 * k.blk + 32 || (k.a & 1)) ++bad[2];
+                        for (int i = k.a; i < k.b; ++i) {
+                            const int u = (w & 3) * kTmemCols + k.tcol + 4 * (i - k.a);
+                            if (k.tcol + 4 * (i - k.a) + 4 > kTmemCols || tmap[u] != k.blk * 4096 + i) ++bad[3];
+                            else tread[u]++;
+                        }
+                        // the column copy masks Kf below iS[j]: only legal if the flag says so
+                        for (int j = 32 * k.blk; j < std::min(N, 32 * k.blk + 32); ++j)
+                            if (t.iS[j] > k.a && !f.colMask) ++bad[2];
+                    }
+                } else if (k.kind == FE_W) {
+                    ++nWtask;
+                } else ++bad[3];
+            }
+        for (int p = 0; p < f.nRowParts; ++p) bad[3] += rpart[p] != 1;
+        for (int p = 0; p < f.nColParts; ++p) bad[3] += cpart[p] != 1;
+        if (nWtask != (N + 31) / 32) ++bad[4];
+        for (int i = 0; i < N; ++i)
+            for (int j = 0; j <= i; ++j) {
+                bad[0] += fbuilt[(size_t)i * N + j] != 1;
+                bad[1] += frow[(size_t)i * N + j] != (j < t.n_bulk[i] ? 1 : 0);
+                bad[2] += fcol[(size_t)i * N + j] != 1;
+            }
+        // band tables: every entry of the host table exactly once, in order, with its stage index
+        long long fent = 0;
+        for (int gh = 0; gh < 2 * f.nwBins; ++gh)
+            for (int e = 0; e < f.bgLen[gh] * 32; ++e) fent += F.bandCoef[f.bgOff[gh] + e] != 0.0;
+        for (int g = 0; g < f.nwBins; ++g)
+            for (int e = 0; e < f.sgLen[g] * 32; ++e) fent += F.bandCoef[f.sgOff[g] + e] != 0.0;
+        long long nz = 0;
+        for (const BandEntry &be : t.band) nz += be.coef != 0.0;
+        if (fent != nz) ++bad[4];
+        for (uint32_t ix : F.bandIdx)
+            if (ix >= (uint32_t)(2 * d.bandD * Np)) ++bad[4];
+        int per[kThreads / 32] = {0};
+        for (int gh = 0; gh < 2 * f.nwBins; ++gh) {
+            if (f.bgWarp[gh] < 0 || f.bgWarp[gh] >= nWarps || ++per[f.bgWarp[gh]] > 2) ++bad[5];
+            if (f.bgLen[gh] & 3) ++bad[5];
+        }
+        if ((size_t)f.off[FO_END] != F.smemDoubles) ++bad[3];
+    }
     for (int q = 0; q < 6; ++q) out[q] = bad[q];
-    out[6] = (long long)S.buildItems.size() + (long long)S.evalItems.size();
+    out[6] = (long long)S.buildItems.size() + (long long)S.evalItems.size()
+             + (long long)F.buildTasks.size() + (long long)F.evalTasks.size();
     out[7] = (long long)(smem_vec_doubles(Np, d.partRowSlots, d.partColSlots, d.nBuildItems + d.nEvalItems, d.bandD)
                          * sizeof(double));
+    return CUDISC_OK;
+}
+
+int cudisc_bins_fast_path(cudisc_bins b, int *on, long long *smem_bytes, int *tmem_cols_used)
+{
+    if (!bins_ok(b)) return fail(CUDISC_ERR_HANDLE, "bad bins handle");
+    Schedule S;
+    build_schedule(b->ht, S);
+    FastSchedule F;
+    build_fast_schedule(b->ht, S, F);
+    if (on) *on = F.f.on;
+    if (smem_bytes) *smem_bytes = F.f.on ? (long long)(F.smemDoubles * sizeof(double)) : 0;
+    if (tmem_cols_used) {
+        int used = 0;
+        if (F.f.on) {
+            used = 4 * fast_binc_cols(F.f.nwBins);
+            for (int gh = 0; gh < 2 * F.f.nwBins; ++gh) used += 3 * F.f.bgLen[gh];
+            for (int g = 0; g < F.f.nwBins; ++g) used += 3 * F.f.sgLen[g];
+            for (uint2 u : F.buildTasks) {
+                const FTask k = ftask_unpack(u);
+                if (k.kind == FB_ROWS && k.tcol != kNoTmem) used += 4 * ((k.b - k.a + 1) & ~1);
+            }
+        }
+        *tmem_cols_used = used;
+    }
     return CUDISC_OK;
 }
 

@@ -62,33 +62,34 @@ struct FSm {
     uint2 *TB, *TE;     // build / evaluation tasks (per-warp lists, FastTables::bw / ew)
 };
 
-__device__ __forceinline__ FSm fast_carve(double *base, const DevTables &tb, const FastTables &ft)
+// offsets (in doubles) of the arrays, computed on the host (FastTables::off): a pointer the compiler
+// has to re-materialise under register pressure costs one add of a kernel parameter
+__device__ __forceinline__ FSm fast_carve(double *base, const FastTables &ft)
 {
     FSm f;
-    const int Np = tb.Np;
-    double *q = base;
-    f.KR = (double2 *)q; q += 2 * (size_t)tb.P;
+    f.KR = (double2 *)base;
     Smem &s = f.s;
-    s.YY = (double2 *)q; q += 2 * Np;
-    s.DTAB = (double2 *)q; q += 2 * Np;
-    s.NN = q; q += Np + 8;
-    s.BANDV = q; q += Np;
-    s.BANDV2 = q; q += Np;
+    s.YY = (double2 *)(base + ft.off[FO_YY]);
+    s.DTAB = (double2 *)(base + ft.off[FO_DTAB]);
+    s.NN = base + ft.off[FO_NN];
+    s.BANDV = base + ft.off[FO_BANDV];
+    s.BANDV2 = base + ft.off[FO_BANDV2];
     s.BINC = nullptr;
-    s.BINI = (int2 *)q; q += Np;
-    s.EXPT = q; q += 64;
-    s.RED = q; q += 96;
+    s.BINI = (int2 *)(base + ft.off[FO_BINI]);
+    s.EXPT = base + ft.off[FO_EXPT];
+    s.RED = base + ft.off[FO_RED];
     s.CTR = nullptr; s.SCHED = nullptr; s.ITB = s.ITE = nullptr;
-    const int nB = ft.bw[16], nE = ft.ew[16];
-    f.TB = (uint2 *)q; f.TE = f.TB + nB; q += (nB + nE + 1) & ~1;
-    s.PARTR = q;
-    s.PARTC = q + (size_t)128 * ft.nRowParts;
-    s.WST = s.PARTC + (size_t)64 * ft.nColParts;
-    double *v = q;
-    s.RI = (double2 *)v; v += 10 * Np;
-    s.B0 = (double2 *)v; v += 2 * Np; s.B1 = (double2 *)v; v += 2 * Np;
-    s.J2 = (double2 *)v; v += 2 * Np; s.J3 = (double2 *)v; v += 2 * Np;
-    s.V5 = v;
+    f.TB = (uint2 *)(base + ft.off[FO_TB]);
+    f.TE = (uint2 *)(base + ft.off[FO_TE]);
+    s.PARTR = base + ft.off[FO_UNION];
+    s.PARTC = base + ft.off[FO_PARTC];
+    s.WST = base + ft.off[FO_WST];
+    s.RI = (double2 *)(base + ft.off[FO_UNION]);
+    s.B0 = (double2 *)(base + ft.off[FO_B0]);
+    s.B1 = (double2 *)(base + ft.off[FO_B1]);
+    s.J2 = (double2 *)(base + ft.off[FO_J2]);
+    s.J3 = (double2 *)(base + ft.off[FO_J3]);
+    s.V5 = base + ft.off[FO_V5];
     return f;
 }
 
@@ -466,7 +467,7 @@ coag_fast_kernel(const DevTables tb, const FastTables ft, const GasArgs gs, cons
     extern __shared__ __align__(16) double smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
     const int N = tb.N, Np = tb.Np;
-    const FSm f = fast_carve(smem_raw, tb, ft);
+    const FSm f = fast_carve(smem_raw, ft);
     const Smem &s = f.s;
     PairConst pc;
     const bool has_vphi = gs.vphi != nullptr;

@@ -58,8 +58,14 @@ __host__ __device__ inline FTask ftask_unpack(uint2 u)
 //            overflow rows), slot = column part p
 //   FE_W     blk = row block whose band products are staged
 
+// shared-memory layout of the fast kernel: offsets in doubles from the start of dynamic shared memory
+// (the K row copy sits at 0).  The build-time role vectors alias the partial-sum slots and the band stage.
+enum { FO_YY = 0, FO_DTAB, FO_NN, FO_BANDV, FO_BANDV2, FO_BINI, FO_EXPT, FO_RED, FO_TB, FO_TE, FO_UNION,
+       FO_PARTC, FO_WST, FO_B0, FO_B1, FO_J2, FO_J3, FO_V5, FO_END, kFastOff };
+
 struct FastTables {
     int on;                        // 0: this mass grid runs on the general kernel
+    int off[kFastOff];             // FO_*: array offsets; off[FO_END] = total doubles
     int bw[17], ew[17];            // warp w: build tasks [bw[w], bw[w+1]), evaluation tasks [ew[w], ew[w+1])
     int colMask;                   // 1: some tensor-memory rows lie below iS[j]: Kf is masked in the column copy
     int nwBins;                    // warps that own bins: ceil(N / 32)
@@ -87,17 +93,22 @@ __host__ __device__ inline int fast_binc_col_r(int warp) { return 16 * (warp >> 
 __host__ __device__ inline int fast_binc_col_c(int nw, int warp) { return 16 * ((nw + 3) >> 2) + 2 * (warp >> 2); }
 __host__ __device__ inline int fast_binc_cols(int nw) { return 16 * ((nw + 3) >> 2) + 2 * (((2 * nw - 1) >> 2) + 1); }
 
-// shared memory of the fast kernel, in doubles, besides the K row copy (2 P doubles)
-__host__ __device__ inline size_t fast_misc_doubles(int Np, int nTasks)
+// fills ft.off from the sizes already set in ft (nRowParts, nColParts, bw, ew)
+inline void fast_layout(FastTables &ft, int P, int Np, int bandD)
 {
-    //      YY  DTAB NN(+8)  BANDV(2) BINI   EXPT RED
-    return (size_t)Np * (2 + 2 + 1 + 2 + 1) + 8 + 64 + 96 + (size_t)((nTasks + 1) & ~1);
-}
-__host__ __device__ inline size_t fast_union_doubles(int Np, int rowParts, int colParts, int bandD)
-{
-    const size_t part = (size_t)128 * rowParts + (size_t)64 * colParts + (size_t)2 * bandD * Np;
-    const size_t build = (size_t)Np * 19;
-    return part > build ? part : build;
+    int q = 2 * P;
+    auto take = [&](int what, int n) { ft.off[what] = q; q += (n + 1) & ~1; };
+    take(FO_YY, 2 * Np); take(FO_DTAB, 2 * Np); take(FO_NN, Np + 8); take(FO_BANDV, Np); take(FO_BANDV2, Np);
+    take(FO_BINI, Np); take(FO_EXPT, 64); take(FO_RED, 96);
+    take(FO_TB, ft.bw[16]); take(FO_TE, ft.ew[16]);
+    ft.off[FO_UNION] = q;
+    ft.off[FO_PARTC] = q + 128 * ft.nRowParts;
+    ft.off[FO_WST] = ft.off[FO_PARTC] + 64 * ft.nColParts;
+    const int part = 128 * ft.nRowParts + 64 * ft.nColParts + 2 * bandD * Np;
+    ft.off[FO_B0] = q + 10 * Np; ft.off[FO_B1] = q + 12 * Np; ft.off[FO_J2] = q + 14 * Np; ft.off[FO_J3] = q + 16 * Np;
+    ft.off[FO_V5] = q + 18 * Np;
+    const int build = 19 * Np;
+    ft.off[FO_END] = q + (part > build ? part : build);
 }
 
 }  // namespace cudisc
