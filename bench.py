@@ -42,6 +42,8 @@ import numpy as np  # noqa: E402
 # add, mul or max each count 1; per-bin hoistable terms excluded).
 I_BUILD = 41      # per pair, once per step: Eqs. 56-62 on a log grid (FP64-pipe instructions of pair_kernel)
 I_EVAL = 6        # per pair per rate evaluation: 4 row-sum + 2 column-sum FMAs
+F_BUILD = 58      # the same formulas counted in flops (FMA = 2, add / mul = 1): 17 FMAs + 24 others
+F_EVAL = 12
 EVALS_PER_STEP = 3
 FP64_LANES_PER_SM = 64
 METRIC = "coagulation cell-updates/sec (FP64 BS3(2) step, kernel built on the fly)"
@@ -164,7 +166,8 @@ def oracle_step_rate(index: int, budget_s: float, warmup: int = 0, steps: int = 
     rate = len(cells) * steps / total
     info = {"cores": threads, "kind": "oracle",
             "sample": f"{len(cells)} of {cfg.n_cells} cells of config {index} ({cfg.n_bins} bins), "
-                      f"{steps} step(s) of oracle orc_step_cells (OpenMP over cells), {total:.1f} s"}
+                      f"{steps} step(s) of oracle orc_step_cells (OpenMP over cells) after {warmup} untimed "
+                      f"step(s) ({'FSAL: 3' if warmup else 'first step: 4'} rate evaluations per step), {total:.1f} s"}
     return rate, info, total / steps
 
 
@@ -324,12 +327,143 @@ def run_ours(args):
             },
         }
         if world == 1 and not args.no_cpu_baseline:
-            rate, info, _ = oracle_step_rate(args.config, budget_s=12.0)
+            rate, info, _ = oracle_step_rate(args.config, budget_s=20.0, warmup=1, steps=1)   # a FSAL step, like the GPU's
             line["cpu_baseline"] = {"value": rate, "unit": "cell-updates/s", **info}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
+    return 0
+
+
+def measured_peaks():
+    """MEASURED_PEAKS.json (driver-written) if present: HBM copy GB/s of this pool's B200s."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+def run_entry(args):
+    """--entry kernel | rates | step_cached | integrate: the other C-ABI entry points on the same workload
+    (config 4 by default), each against its own roof: FP64 issue slots for `kernel`, HBM
+    for `rates` / `step_cached` (16 B per pair read); `integrate` = BASELINE.json config 4 as stated
+    (1000 accepted adaptive steps: time to solution and mass drift)."""
+    import torch
+
+    import paper_2402_18471_b200 as cd
+    from paper_2402_18471_b200 import synth_disc
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+    dev = torch.device("cuda", env_int("LOCAL_RANK", 0))
+    torch.cuda.set_device(dev)
+    cfg = synth_disc.CONFIGS[args.config]
+    full = args.entry == "integrate"
+    n_cells = cfg.n_cells if full else min(cfg.n_cells, args.cells)
+    cells = None if n_cells == cfg.n_cells else np.arange(n_cells)        # the first n_cells cells of the grid
+    d = synth_disc.make_disc(args.config, cells=cells)
+    C, N, P = d.n_cells, d.n_bins, cfg.n_pairs
+    pc = cd.Params(mu=cfg.mu, v_frag=cfg.v_frag, alpha=cfg.alpha, eta=cfg.eta, chi_im=cfg.chi_im,
+                   sigma_mol=cfg.sigma_mol)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    gas = dict(T=t(d.T), rho_gas=t(d.rho_gas), Omega=t(d.Omega), v_R=t(d.v_R), v_Z=t(d.v_Z), alpha=t(d.alpha))
+    bins = cd.Bins(N, d.a_min, d.a_max, d.rho_m, pc)
+    grid = cd.Grid(cfg.n_r, cfg.n_z, bins) if full else cd.Grid(C, 1, bins)
+    grid.bind_gas(**gas)
+    dt = load_dt(args.config)
+    rho = t(d.rho_dust)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    dfma_per_s, _ = cd.cudisc_microbench_dfma(0)
+    copy_bps, _ = cd.cudisc_microbench_copy(1 << 30)
+    peaks = measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs") or copy_bps / 1e9)
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs" if peaks.get("hbm_gbs") else "in-process copy microbenchmark"
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    sampler = ClockSampler(dev.index or 0)
+    n0 = cd.cudisc_launch_count()
+    base = {"entry": args.entry, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "dtype": "f64",
+            "data": "synthetic", "higher_is_better": True, "vs_baseline": None,
+            "config": {"workload": f"BASELINE.json config {cfg.index}: {C} of {cfg.n_cells} cells, {N} bins",
+                       "n_cells": C, "n_bins": N, "pairs_per_cell": P,
+                       "l2": "flushed between timed launches (256 MiB memset outside the event pair)"}}
+
+    if args.entry == "integrate":
+        m0 = rho.sum(dim=1)
+        torch.cuda.synchronize()
+        sampler.start()
+        t0 = time.perf_counter()
+        info, log = cd.cudisc_coag_integrate_steps(grid, bins, rho, args.accepted, dt, max_steps=4 * args.accepted)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        sampler.stop()
+        drift = float(((rho.sum(dim=1) - m0).abs() / m0).max())
+        line = dict(base, metric="time to solution of 1000 accepted adaptive BS3(2) steps (cudisc_coag_integrate)",
+                    value=wall, unit="s", higher_is_better=False,
+                    n_accepted=info["n_accepted"], n_rejected=info["n_rejected"], t_done_s=info["t_done"],
+                    dt_last_s=info["dt_last"], mass_drift_rel_max=drift,
+                    mass_drift_per_accepted_step=drift / max(info["n_accepted"], 1),
+                    cell_updates_per_s=C * (info["n_accepted"] + info["n_rejected"]) / wall,
+                    min_rho=float(rho.min()), clocks=sampler.summary(),
+                    gpu_launches=int(cd.cudisc_launch_count() - n0))
+        print(json.dumps(line), flush=True)
+        return 0
+
+    K = torch.empty((C, 2, P), dtype=torch.float64, device=dev)
+    cd.cudisc_coag_kernel(grid, bins, gas, pc, K)
+    out = torch.empty_like(rho)
+    err = torch.empty(C, dtype=torch.float64, device=dev)
+
+    def launch():
+        if args.entry == "kernel":
+            cd.cudisc_coag_kernel(grid, bins, gas, pc, K)
+        elif args.entry == "rates":
+            cd.cudisc_coag_rates(grid, bins, K, rho, out)
+        else:
+            cd.cudisc_coag_step_cached(grid, bins, K, rho, dt, err)
+
+    for _ in range(args.warmup):
+        launch()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    sampler.start()
+    for e0, e1 in ev:
+        flush.zero_()
+        e0.record(stream)
+        launch()
+        e1.record(stream)
+    torch.cuda.synchronize()
+    sampler.stop()
+    sec = statistics.mean(e0.elapsed_time(e1) for e0, e1 in ev) * 1e-3
+    pairs = float(C) * P
+    evals = {"kernel": 0, "rates": 1, "step_cached": EVALS_PER_STEP}[args.entry]
+    hbm_bytes = 16.0 * pairs + (2 if args.entry == "rates" else 6 if args.entry == "step_cached" else 0) * 8.0 * C * N
+    gbs = hbm_bytes / sec / 1e9
+    alu_instr = pairs * (I_BUILD if args.entry == "kernel" else evals * I_EVAL)
+    alu_frac = alu_instr / sec / (sm_count * FP64_LANES_PER_SM * (sampler.summary().get("sm_max_mhz") or 1965) * 1e6)
+    hbm_frac = gbs / hbm_peak
+    bound = "alu" if (args.entry == "kernel" and alu_frac > hbm_frac) else "hbm"
+    line = dict(base, metric={"kernel": "kernel pairs/s (cudisc_coag_kernel, K written to HBM)",
+                              "rates": "rate-evaluation pairs/s (cudisc_coag_rates, K read from HBM)",
+                              "step_cached": "cell-updates/s (cudisc_coag_step_cached, K read from HBM)"}[args.entry],
+                value=(C / sec) if args.entry == "step_cached" else pairs * max(evals, 1) / sec,
+                unit="cell-updates/s" if args.entry == "step_cached" else "pairs/s", ms_per_launch=1e3 * sec,
+                clocks=sampler.summary(), gpu_launches=int(cd.cudisc_launch_count() - n0),
+                roofline={"bound": bound,
+                          "achieved": gbs if bound == "hbm" else 2.0 * alu_instr / sec / 1e12,
+                          "peak": hbm_peak if bound == "hbm" else 2.0 * sm_count * FP64_LANES_PER_SM * 1965e6 / 1e12,
+                          "unit": "GB/s" if bound == "hbm" else "TFLOP/s",
+                          "frac": hbm_frac if bound == "hbm" else alu_frac, "traffic": None,
+                          "hbm_gbs": gbs, "hbm_frac": hbm_frac, "alu_frac": alu_frac,
+                          "how": f"algorithmic HBM bytes per launch = 16 B x {pairs:.4g} pairs (+ the [C x N] arrays) "
+                                 f"= {hbm_bytes:.4g} / mean CUDA-event launch duration {1e3 * sec:.3f} ms; HBM peak "
+                                 f"{hbm_peak:.0f} GB/s from {hbm_src}; alu_frac = FP64 instructions of the minimal "
+                                 f"formulas / (SMs x 64 lanes x max clock)",
+                          "hbm_copy_measured_gbs": copy_bps / 1e9,
+                          "peak_measured_dfma_tflops": 2.0 * dfma_per_s / 1e12})
+    print(json.dumps(line), flush=True)
     return 0
 
 
@@ -341,10 +475,16 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--entry", choices=["step", "kernel", "rates", "step_cached", "integrate"], default="step",
+                    help="C-ABI entry point to time (default: cudisc_coag_step, the contract line)")
+    ap.add_argument("--cells", type=int, default=16000, help="cells of the workload for --entry kernel/rates/step_cached")
+    ap.add_argument("--accepted", type=int, default=1000, help="accepted steps of --entry integrate")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    if args.entry != "step":
+        return run_entry(args)
     return run_ours(args)
 
 

@@ -182,7 +182,10 @@ int cudisc_coag_rates_otf(cudisc_grid g, cudisc_bins b, const double *rho_dust, 
  *   E_c = max_k |e_k| / (atol_factor * sum_k rho_k + rtol * max(|rho_k|, |rho_k^new|))   (R10);
  * the step is accepted by the caller iff max_c E_c <= 1 (this call always advances rho_dust).
  * The first call after create / bind_gas / reset_fsal evaluates k1 = f(rho) (4 rate evaluations);
- * later calls reuse the saved k4 (FSAL, 3 evaluations). */
+ * later calls reuse the saved k4 (FSAL, 3 evaluations) -- only for the same rho_dust array (a different
+ * pointer, or a switch between this call and cudisc_coag_step_cached, recomputes k1); call
+ * cudisc_grid_reset_fsal after modifying rho_dust in place.  One device per process is assumed for a
+ * given handle: tables and scratch live on the device that was current at cudisc_grid_create. */
 int cudisc_coag_step(cudisc_grid g, cudisc_bins b, double *rho_dust, double dt,
                      double *err_out, cudisc_stream stream);
 
@@ -226,17 +229,29 @@ double cudisc_controller_next_dt(double E, double h);
 
 /* Integrates every cell over t_span seconds with adaptive BS3(2) sub-steps of ONE global size
  * (coagulation sub-cycles inside the global step with the gas state frozen).
- * Each trial step is one cudisc_coag_step launch into trial buffers owned by g, a max-reduction of
- * the per-cell error norms on the device and an 8-byte read-back; rejected steps leave the state
- * untouched.  The last step is cut to land on t_span.
+ * The controller runs on the DEVICE: every trial is one step launch that reads its size and
+ * its buffer roles from a controller state in device memory, followed by a one-block kernel that reduces
+ * the per-cell error norms, accepts or rejects, and writes the next size; trials are enqueued in batches
+ * of 32 without a host round trip (launches after the end return at once) and the host reads the state
+ * once per batch.  Rejected steps leave the state untouched.  The last step is cut to land on t_span.
  * rho_dust: DEVICE [C x N] in/out.  dt_try: first trial size, s (> 0).  max_steps: bound on accepted
  * + rejected steps.  dt_log: HOST [max_steps] or NULL; receives the size of every trial step in
  * order, negated when the step was rejected.  info: HOST, may be NULL.
- * SYNCHRONISES with `stream` (once per trial step).  A non-finite error norm stops the
- * integration with CUDISC_ERR_INVALID (rho_dust then holds the last accepted state). */
+ * SYNCHRONISES with `stream` (once per batch).  Buffers owned by g are allocated on the first call, all or
+ * nothing.  A non-finite error norm stops the integration with CUDISC_ERR_INVALID (rho_dust then holds
+ * the last accepted state).
+ * FSAL: the saved derivative is reused only if it was produced from this same rho_dust array with the
+ * kernel built on the fly (the library remembers both); after rho_dust was modified IN PLACE by the caller
+ * (dust transport between coagulation calls) cudisc_grid_reset_fsal must be called. */
 int cudisc_coag_integrate(cudisc_grid g, cudisc_bins b, double *rho_dust, double t_span, double dt_try,
                           int max_steps, double *dt_log, cudisc_integrate_info *info,
                           cudisc_stream stream);
+
+/* Same, but stops after n_accepted accepted steps instead of at a time (BASELINE.json config 4:
+ * "integrate 1000 coagulation steps"); info->t_done is the time reached. */
+int cudisc_coag_integrate_steps(cudisc_grid g, cudisc_bins b, double *rho_dust, int n_accepted, double dt_try,
+                                int max_steps, double *dt_log, cudisc_integrate_info *info,
+                                cudisc_stream stream);
 
 /* ---------------------------------------------------------------------------------------------
  * Roofline denominators measured in the same process (north_star: "peaks measured by a

@@ -45,7 +45,7 @@ EXPORTS = [
     "cudisc_bins_create", "cudisc_bins_create_general", "cudisc_bins_destroy", "cudisc_bins_query",
     "cudisc_bins_expand_outcomes", "cudisc_bins_schedule_check", "cudisc_bins_fast_path", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
     "cudisc_grid_destroy", "cudisc_coag_kernel", "cudisc_coag_rates", "cudisc_coag_rates_otf",
-    "cudisc_coag_step", "cudisc_coag_step_cached", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_controller_next_dt",
+    "cudisc_coag_step", "cudisc_coag_step_cached", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_coag_integrate_steps", "cudisc_controller_next_dt",
     "cudisc_microbench_dfma",
     "cudisc_microbench_copy", "cudisc_launch_count", "cudisc_last_error", "cudisc_version",
 ]
@@ -81,6 +81,8 @@ def lib() -> C.CDLL:
         L.cudisc_coag_step_cached.argtypes = [vp, vp, vp, vp, C.c_double, vp, vp]
         L.cudisc_coag_integrate.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int, dp,
                                             C.POINTER(cudisc_integrate_info), vp]
+        L.cudisc_coag_integrate_steps.argtypes = [vp, vp, vp, C.c_int, C.c_double, C.c_int, dp,
+                                                  C.POINTER(cudisc_integrate_info), vp]
         L.cudisc_controller_next_dt.argtypes = [C.c_double, C.c_double]
         L.cudisc_controller_next_dt.restype = C.c_double
         L.cudisc_microbench_dfma.argtypes = [C.c_int, dp, dp]
@@ -310,6 +312,12 @@ def cudisc_controller_next_dt(E: float, h: float) -> float:
     return float(lib().cudisc_controller_next_dt(float(E), float(h)))
 
 
+def _info_dict(info, log):
+    n = info.n_accepted + info.n_rejected
+    return ({"t_done": info.t_done, "dt_last": info.dt_last, "dt_next": info.dt_next, "err_last": info.err_last,
+             "n_accepted": info.n_accepted, "n_rejected": info.n_rejected}, log[:n].copy())
+
+
 def cudisc_coag_integrate(grid: Grid, bins: Bins, rho_dust, t_span: float, dt_try: float, max_steps: int = 10000,
                           stream=None):
     """Adaptive BS3(2) sub-cycling over t_span.  Returns (info dict, dt_log): dt_log holds
@@ -320,9 +328,20 @@ def cudisc_coag_integrate(grid: Grid, bins: Bins, rho_dust, t_span: float, dt_tr
     _check(lib().cudisc_coag_integrate(grid.handle, bins.handle, _dev_ptr(rho_dust, "rho_dust", Cn * N),
                                        float(t_span), float(dt_try), int(max_steps),
                                        log.ctypes.data_as(C.POINTER(C.c_double)), C.byref(info), _stream(stream)))
-    n = info.n_accepted + info.n_rejected
-    return ({"t_done": info.t_done, "dt_last": info.dt_last, "dt_next": info.dt_next, "err_last": info.err_last,
-             "n_accepted": info.n_accepted, "n_rejected": info.n_rejected}, log[:n].copy())
+    return _info_dict(info, log)
+
+
+def cudisc_coag_integrate_steps(grid: Grid, bins: Bins, rho_dust, n_accepted: int, dt_try: float,
+                                max_steps: int = 10000, stream=None):
+    """Adaptive sub-cycling until n_accepted steps were accepted (BASELINE.json config 4)."""
+    Cn, N = grid.n_cells, bins.n_bins
+    log = np.zeros(max_steps)
+    info = cudisc_integrate_info()
+    _check(lib().cudisc_coag_integrate_steps(grid.handle, bins.handle, _dev_ptr(rho_dust, "rho_dust", Cn * N),
+                                             int(n_accepted), float(dt_try), int(max_steps),
+                                             log.ctypes.data_as(C.POINTER(C.c_double)), C.byref(info),
+                                             _stream(stream)))
+    return _info_dict(info, log)
 
 
 def cudisc_microbench_dfma(n_iter: int = 0):

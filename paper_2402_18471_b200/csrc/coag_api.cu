@@ -64,12 +64,16 @@ struct cudisc_grid_s {
     bool gas_bound;
     cudisc_gas_state gs;
     bool fsal_valid;
+    const void *fsal_rho, *fsal_K;   // the state array (and kernel planes, NULL = built on the fly) k_fsal belongs to
     double *k_fsal;     // [C x N]
     double *kslab;      // per-CTA overflow of the K store
     double *stage_rho;  // [C x N] staging of cudisc_coag_step_host (lazy)
     double *stage_err;  // [C]
-    double *trial_rho, *trial_k, *trial_err, *d_emax;   // cudisc_coag_integrate (lazy)
-    double *h_emax;     // pinned host scalar
+    cudaStream_t pipe[2];      // internal streams of the sliced end-to-end step
+    cudaEvent_t pipe_ev[3];
+    double *trial_rho, *trial_k, *trial_err, *d_log;   // cudisc_coag_integrate (lazy, all or nothing)
+    CtrlState *d_ctrl, *h_ctrl;                        // controller state: device, pinned host mirror
+    int log_cap;
     long long *prof;    // CUDISC_PROF builds only
     int num_sms, smem_optin, grid_ctas, Psm, smem_bytes;
     bool fast;          // cudisc_coag_step / rates_otf run on the tensor-memory kernel
@@ -620,18 +624,31 @@ int check_pair(cudisc_grid g, cudisc_bins b)
     return CUDISC_OK;
 }
 
-int run(cudisc_grid g, int mode, const GasArgs &ga, StepArgs sa, cudisc_stream stream)
+// Launch over the cells [c0, c1) of the grid (default: all): cells are independent, so a range is the same
+// launch with every per-cell pointer advanced by c0.
+int run(cudisc_grid g, int mode, GasArgs ga, StepArgs sa, cudisc_stream stream, int c0 = 0, int c1 = -1)
 {
     int rc = upload_tables(g->bins);
     if (rc) return rc;
-    sa.C = g->C;
+    if (c1 < 0) c1 = g->C;
+    sa.C = c1 - c0;
+    if (c0 > 0) {
+        const size_t N = (size_t)g->bins->ht.N, P2 = 2 * (size_t)g->bins->dt.P;
+        auto adv = [&](const double *&p, size_t stride) { if (p) p += (size_t)c0 * stride; };
+        auto advw = [&](double *&p, size_t stride) { if (p) p += (size_t)c0 * stride; };
+        adv(ga.T, 1); adv(ga.rho_g, 1); adv(ga.Omega, 1); adv(ga.alpha, 1);
+        adv(ga.vR, N); adv(ga.vZ, N); adv(ga.vphi, N); adv(ga.hd, N);
+        adv(sa.rho, N); adv(sa.k_fsal, N); advw(sa.rho_out, N); advw(sa.k_out, N); advw(sa.err, 1);
+        adv(sa.Kin, P2);
+        if (sa.out) sa.out += (size_t)c0 * (mode == MODE_KERNEL ? P2 : N);
+    }
     sa.Psm = g->Psm;
     sa.kslab = g->kslab;
     sa.prof = g->prof;
-    LaunchCfg lc{g->grid_ctas, g->smem_bytes, g->smem_optin};
+    LaunchCfg lc{std::min(g->grid_ctas, std::max(1, sa.C)), g->smem_bytes, g->smem_optin};
     cudaError_t e;
     if (g->fast && (mode == MODE_OTF || mode == MODE_STEP) && !ga.hd) {
-        LaunchCfg lf{g->fast_ctas, (int)g->bins->fast_smem_bytes, g->smem_optin};
+        LaunchCfg lf{std::min(g->fast_ctas, std::max(1, sa.C)), (int)g->bins->fast_smem_bytes, g->smem_optin};
         e = launch_fast(mode, lf, g->bins->dt, g->bins->ft, ga, sa, (cudaStream_t)stream);
     } else {
         e = launch_cells(mode, lc, g->bins->dt, ga, sa, (cudaStream_t)stream);
@@ -991,9 +1008,13 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
     g->n_r = n_r; g->n_z = n_z; g->C = n_r * n_z;
     g->bins = b;
     g->gas_bound = false; g->fsal_valid = false;
+    g->fsal_rho = g->fsal_K = nullptr;
     g->k_fsal = nullptr; g->kslab = nullptr;
     g->stage_rho = nullptr; g->stage_err = nullptr; g->prof = nullptr;
-    g->trial_rho = g->trial_k = g->trial_err = g->d_emax = g->h_emax = nullptr;
+    g->pipe[0] = g->pipe[1] = nullptr;
+    g->pipe_ev[0] = g->pipe_ev[1] = g->pipe_ev[2] = nullptr;
+    g->trial_rho = g->trial_k = g->trial_err = g->d_log = nullptr;
+    g->d_ctrl = nullptr; g->h_ctrl = nullptr; g->log_cap = 0;
     g->num_sms = sms; g->smem_optin = optin;
 
     const DevTables &d = b->dt;
@@ -1065,12 +1086,15 @@ int cudisc_grid_destroy(cudisc_grid g)
     if (g->kslab) cudaFree(g->kslab);
     if (g->stage_rho) cudaFree(g->stage_rho);
     if (g->stage_err) cudaFree(g->stage_err);
+    for (int q = 0; q < 2; ++q) if (g->pipe[q]) cudaStreamDestroy(g->pipe[q]);
+    for (int q = 0; q < 3; ++q) if (g->pipe_ev[q]) cudaEventDestroy(g->pipe_ev[q]);
     if (g->prof) cudaFree(g->prof);
     if (g->trial_rho) cudaFree(g->trial_rho);
     if (g->trial_k) cudaFree(g->trial_k);
     if (g->trial_err) cudaFree(g->trial_err);
-    if (g->d_emax) cudaFree(g->d_emax);
-    if (g->h_emax) cudaFreeHost(g->h_emax);
+    if (g->d_ctrl) cudaFree(g->d_ctrl);
+    if (g->d_log) cudaFree(g->d_log);
+    if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
     g->magic = 0;
     delete g;
     return CUDISC_OK;
@@ -1132,9 +1156,11 @@ int cudisc_coag_step(cudisc_grid g, cudisc_bins b, double *rho_dust, double dt, 
     sa.k_fsal = g->k_fsal; sa.k_out = g->k_fsal;
     sa.err = err_out;
     sa.dt = dt; sa.rtol = b->p.rtol; sa.atol_factor = b->p.atol_factor;
+    // the saved derivative belongs to one state array and one kernel source: anything else recomputes k1
+    if (g->fsal_rho != rho_dust || g->fsal_K != nullptr) g->fsal_valid = false;
     sa.have_k1 = g->fsal_valid ? 1 : 0;
     rc = run(g, 3, gas_args(g->gs, b->p), sa, stream);
-    if (rc == CUDISC_OK) g->fsal_valid = true;
+    if (rc == CUDISC_OK) { g->fsal_valid = true; g->fsal_rho = rho_dust; g->fsal_K = nullptr; }
     return rc;
 }
 
@@ -1151,11 +1177,12 @@ int cudisc_coag_step_cached(cudisc_grid g, cudisc_bins b, const double *K, doubl
     sa.k_fsal = g->k_fsal; sa.k_out = g->k_fsal;
     sa.err = err_out;
     sa.dt = dt; sa.rtol = b->p.rtol; sa.atol_factor = b->p.atol_factor;
+    if (g->fsal_rho != rho_dust || g->fsal_K != K) g->fsal_valid = false;
     sa.have_k1 = g->fsal_valid ? 1 : 0;
     GasArgs ga;
     memset(&ga, 0, sizeof(ga));
     rc = run(g, 4, ga, sa, stream);
-    if (rc == CUDISC_OK) g->fsal_valid = true;
+    if (rc == CUDISC_OK) { g->fsal_valid = true; g->fsal_rho = rho_dust; g->fsal_K = K; }
     return rc;
 }
 
@@ -1164,27 +1191,68 @@ int cudisc_coag_step_host(cudisc_grid g, cudisc_bins b, double *rho_host, double
 {
     int rc = check_pair(g, b);
     if (rc) return rc;
+    if (!g->gas_bound) return fail(CUDISC_ERR_INVALID, "no gas state bound (cudisc_grid_bind_gas)");
     if (!rho_host || !err_host) return fail(CUDISC_ERR_INVALID, "NULL array argument");
-    const size_t row_bytes = (size_t)g->C * b->ht.N * sizeof(double);
+    const size_t N = (size_t)b->ht.N;
+    const size_t row_bytes = (size_t)g->C * N * sizeof(double);
     const size_t err_bytes = (size_t)g->C * sizeof(double);
     cudaError_t e = cudaSuccess;
-    if (!g->stage_rho) {
+    if (!g->stage_rho) {                           // all or nothing
         e = cudaMalloc((void **)&g->stage_rho, row_bytes);
         if (e == cudaSuccess) e = cudaMalloc((void **)&g->stage_err, err_bytes);
+        for (int q = 0; q < 2 && e == cudaSuccess; ++q) e = cudaStreamCreateWithFlags(&g->pipe[q], cudaStreamNonBlocking);
+        for (int q = 0; q < 3 && e == cudaSuccess; ++q) e = cudaEventCreateWithFlags(&g->pipe_ev[q], cudaEventDisableTiming);
         if (e != cudaSuccess) {
-            if (g->stage_rho) { cudaFree(g->stage_rho); g->stage_rho = nullptr; }
-            return cuda_fail(e, "cudaMalloc(staging)");
+            if (g->stage_rho) cudaFree(g->stage_rho);
+            if (g->stage_err) cudaFree(g->stage_err);
+            for (int q = 0; q < 2; ++q) if (g->pipe[q]) { cudaStreamDestroy(g->pipe[q]); g->pipe[q] = nullptr; }
+            for (int q = 0; q < 3; ++q) if (g->pipe_ev[q]) { cudaEventDestroy(g->pipe_ev[q]); g->pipe_ev[q] = nullptr; }
+            g->stage_rho = g->stage_err = nullptr;
+            return cuda_fail(e, "staging buffers / streams");
         }
     }
+    // Cells are independent: the grid is cut in slices that alternate between two internal streams, so the
+    // host->device copy of slice s + 1 and the device->host copy of slice s - 1 run under the kernel of
+    // slice s (copy engines and SMs in parallel).  Both streams start after `stream` and `stream` waits
+    // for both.
     cudaStream_t st = (cudaStream_t)stream;
-    e = cudaMemcpyAsync(g->stage_rho, rho_host, row_bytes, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(H2D)");
-    rc = cudisc_coag_step(g, b, g->stage_rho, dt, g->stage_err, stream);
-    if (rc) return rc;
-    e = cudaMemcpyAsync(rho_host, g->stage_rho, row_bytes, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(err_host, g->stage_err, err_bytes, cudaMemcpyDeviceToHost, st);
+    if (g->fsal_rho != g->stage_rho || g->fsal_K != nullptr) g->fsal_valid = false;
+    StepArgs sa;
+    memset(&sa, 0, sizeof(sa));
+    sa.rho = g->stage_rho; sa.rho_out = g->stage_rho;
+    sa.k_fsal = g->k_fsal; sa.k_out = g->k_fsal;
+    sa.err = g->stage_err;
+    sa.dt = dt; sa.rtol = b->p.rtol; sa.atol_factor = b->p.atol_factor;
+    sa.have_k1 = g->fsal_valid ? 1 : 0;
+    const GasArgs ga = gas_args(g->gs, b->p);
+    const int min_cells = 8 * g->num_sms;                        // keep every SM busy within a slice
+    // (the per-CTA overflow slab of the general kernel is indexed by CTA: no two launches in flight then)
+    const int n_slices = g->kslab ? 1 : std::max(1, std::min(4, g->C / std::max(1, min_cells)));
+    e = cudaEventRecord(g->pipe_ev[0], st);
+    for (int q = 0; q < 2 && e == cudaSuccess; ++q) e = cudaStreamWaitEvent(g->pipe[q], g->pipe_ev[0], 0);
+    if (e != cudaSuccess) return cuda_fail(e, "step_host fork");
+    for (int sl = 0; sl < n_slices; ++sl) {
+        const int c0 = (int)((long long)g->C * sl / n_slices), c1 = (int)((long long)g->C * (sl + 1) / n_slices);
+        cudaStream_t ps = g->pipe[sl & 1];
+        e = cudaMemcpyAsync(g->stage_rho + (size_t)c0 * N, rho_host + (size_t)c0 * N,
+                            (size_t)(c1 - c0) * N * sizeof(double), cudaMemcpyHostToDevice, ps);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(H2D)");
+        rc = run(g, MODE_STEP, ga, sa, (cudisc_stream)ps, c0, c1);
+        if (rc) return rc;
+        e = cudaMemcpyAsync(rho_host + (size_t)c0 * N, g->stage_rho + (size_t)c0 * N,
+                            (size_t)(c1 - c0) * N * sizeof(double), cudaMemcpyDeviceToHost, ps);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(err_host + c0, g->stage_err + c0, (size_t)(c1 - c0) * sizeof(double),
+                                cudaMemcpyDeviceToHost, ps);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(D2H)");
+    }
+    for (int q = 0; q < 2 && e == cudaSuccess; ++q) {
+        e = cudaEventRecord(g->pipe_ev[1 + q], g->pipe[q]);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, g->pipe_ev[1 + q], 0);
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return cuda_fail(e, "step_host copies");
+    if (e != cudaSuccess) return cuda_fail(e, "step_host join");
+    g->fsal_valid = true; g->fsal_rho = g->stage_rho; g->fsal_K = nullptr;
     return CUDISC_OK;
 }
 
@@ -1196,6 +1264,108 @@ double cudisc_controller_next_dt(double E, double h)
     return h * f;
 }
 
+}  // extern "C"
+
+namespace {
+
+void free_integrate(cudisc_grid g)
+{
+    if (g->trial_rho) cudaFree(g->trial_rho);
+    if (g->trial_k) cudaFree(g->trial_k);
+    if (g->trial_err) cudaFree(g->trial_err);
+    if (g->d_ctrl) cudaFree(g->d_ctrl);
+    if (g->d_log) cudaFree(g->d_log);
+    if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
+    g->trial_rho = g->trial_k = g->trial_err = g->d_log = nullptr;
+    g->d_ctrl = nullptr; g->h_ctrl = nullptr;
+    g->log_cap = 0;
+}
+
+// Adaptive sub-cycling driven from the device: every trial is one step launch that reads its
+// size and buffer roles from the controller state, plus one controller launch; trials are enqueued in
+// batches of kBatch without a host round trip (launches after the end are no-ops) and the host reads the
+// 96-byte state once per batch.
+int integrate_impl(cudisc_grid g, cudisc_bins b, double *rho_dust, double t_span, int max_accepted,
+                   double dt_try, int max_steps, double *dt_log, cudisc_integrate_info *info,
+                   cudisc_stream stream)
+{
+    constexpr int kBatch = 32;
+    const size_t row_bytes = (size_t)g->C * b->ht.N * sizeof(double);
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaSuccess;
+    if (!g->trial_rho || g->log_cap < max_steps) {
+        free_integrate(g);                  // all or nothing: a partial failure leaves no dangling pointer
+        e = cudaMalloc((void **)&g->trial_rho, row_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g->trial_k, row_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g->trial_err, (size_t)g->C * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g->d_ctrl, sizeof(CtrlState));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g->d_log, (size_t)max_steps * sizeof(double));
+        if (e == cudaSuccess) e = cudaMallocHost((void **)&g->h_ctrl, sizeof(CtrlState));
+        if (e != cudaSuccess) { free_integrate(g); return cuda_fail(e, "cudaMalloc(integrate)"); }
+        g->log_cap = max_steps;
+    }
+    CtrlState c;
+    memset(&c, 0, sizeof(c));
+    c.t = 0.0; c.t_span = t_span; c.dt = dt_try;
+    c.cut = dt_try >= t_span; c.h = c.cut ? t_span : dt_try;
+    if (g->fsal_rho != rho_dust || g->fsal_K != nullptr) g->fsal_valid = false;
+    c.cur = 0; c.have_k1 = g->fsal_valid ? 1 : 0;
+    c.max_acc = max_accepted; c.max_steps = max_steps;
+    *g->h_ctrl = c;
+    e = cudaMemcpyAsync(g->d_ctrl, g->h_ctrl, sizeof(CtrlState), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);       // h_ctrl is reused for the read-backs
+    if (e != cudaSuccess) return cuda_fail(e, "integrate setup");
+
+    StepArgs sa;
+    memset(&sa, 0, sizeof(sa));
+    sa.rho = rho_dust; sa.rho_out = g->trial_rho;           // buffer pair 0 / 1 (roles swap with ctrl->cur)
+    sa.k_fsal = g->k_fsal; sa.k_out = g->trial_k;
+    sa.err = g->trial_err;
+    sa.rtol = b->p.rtol; sa.atol_factor = b->p.atol_factor;
+    sa.ctrl = g->d_ctrl;
+    const GasArgs ga = gas_args(g->gs, b->p);
+    int enq = 0;
+    for (;;) {
+        const int n = std::min(kBatch, max_steps - enq);
+        for (int q = 0; q < n; ++q) {
+            int rc = run(g, MODE_STEP, ga, sa, stream);
+            if (rc) return rc;
+            e = launch_ctrl(g->trial_err, g->C, g->d_ctrl, g->d_log, st);
+            if (e != cudaSuccess) return cuda_fail(e, "controller launch");
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+        }
+        enq += n;
+        e = cudaMemcpyAsync(g->h_ctrl, g->d_ctrl, sizeof(CtrlState), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "integrate batch");
+        if (g->h_ctrl->done || enq >= max_steps) break;
+    }
+    c = *g->h_ctrl;
+    const int n_trials = c.n_acc + c.n_rej;
+    if (dt_log && n_trials > 0) {
+        e = cudaMemcpyAsync(dt_log, g->d_log, (size_t)n_trials * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "integrate log copy");
+    }
+    if (c.cur) {                                            // state ended in the second buffer pair
+        e = cudaMemcpyAsync(rho_dust, g->trial_rho, row_bytes, cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "integrate copy-back");
+        std::swap(g->k_fsal, g->trial_k);
+    }
+    if (c.n_acc > 0) { g->fsal_valid = true; g->fsal_rho = rho_dust; g->fsal_K = nullptr; }
+    if (info) {
+        info->t_done = c.t; info->dt_last = c.dt_last; info->dt_next = c.dt; info->err_last = c.err_last;
+        info->n_accepted = c.n_acc; info->n_rejected = c.n_rej;
+    }
+    if (c.status) return fail(CUDISC_ERR_INVALID, "non-finite error norm at t = %g s (dt = %g s)", c.t, c.h);
+    return CUDISC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int cudisc_coag_integrate(cudisc_grid g, cudisc_bins b, double *rho_dust, double t_span, double dt_try,
                           int max_steps, double *dt_log, cudisc_integrate_info *info, cudisc_stream stream)
 {
@@ -1205,69 +1375,19 @@ int cudisc_coag_integrate(cudisc_grid g, cudisc_bins b, double *rho_dust, double
     if (!rho_dust) return fail(CUDISC_ERR_INVALID, "NULL array argument");
     if (!(t_span > 0.0) || !(dt_try > 0.0) || max_steps < 1)
         return fail(CUDISC_ERR_INVALID, "need t_span > 0, dt_try > 0, max_steps >= 1");
-    const size_t row_bytes = (size_t)g->C * b->ht.N * sizeof(double);
-    cudaError_t e = cudaSuccess;
-    if (!g->trial_rho) {
-        e = cudaMalloc((void **)&g->trial_rho, row_bytes);
-        if (e == cudaSuccess) e = cudaMalloc((void **)&g->trial_k, row_bytes);
-        if (e == cudaSuccess) e = cudaMalloc((void **)&g->trial_err, (size_t)g->C * sizeof(double));
-        if (e == cudaSuccess) e = cudaMalloc((void **)&g->d_emax, sizeof(double));
-        if (e == cudaSuccess) e = cudaMallocHost((void **)&g->h_emax, sizeof(double));
-        if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(integrate)");
-    }
-    cudaStream_t st = (cudaStream_t)stream;
-    double *cur = rho_dust, *alt = g->trial_rho;        // state ping-pong; the FSAL buffers swap with it
-    double t = 0.0, dt = dt_try, dt_last = 0.0, err_last = 0.0;
-    int n_acc = 0, n_rej = 0, status = CUDISC_OK;
-    while (t < t_span && n_acc + n_rej < max_steps) {
-        const double left = t_span - t;
-        const bool cut = dt >= left;
-        const double h = cut ? left : dt;
-        StepArgs sa;
-        memset(&sa, 0, sizeof(sa));
-        sa.rho = cur; sa.rho_out = alt;
-        sa.k_fsal = g->k_fsal; sa.k_out = g->trial_k;
-        sa.err = g->trial_err;
-        sa.dt = h; sa.rtol = b->p.rtol; sa.atol_factor = b->p.atol_factor;
-        sa.have_k1 = g->fsal_valid ? 1 : 0;
-        rc = run(g, 3, gas_args(g->gs, b->p), sa, stream);
-        if (rc) return rc;
-        e = launch_err_max(g->trial_err, g->C, g->d_emax, st);
-        g_launches.fetch_add(1, std::memory_order_relaxed);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(g->h_emax, g->d_emax, sizeof(double), cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        if (e != cudaSuccess) return cuda_fail(e, "integrate step");
-        const double E = *g->h_emax;
-        if (!(E == E) || std::isinf(E)) {
-            status = fail(CUDISC_ERR_INVALID, "non-finite error norm at t = %g s (dt = %g s)", t, h);
-            break;
-        }
-        if (E <= 1.0) {                                 // accept
-            std::swap(cur, alt);
-            std::swap(g->k_fsal, g->trial_k);
-            g->fsal_valid = true;
-            t = cut ? t_span : t + h;
-            dt_last = h; err_last = E;
-            if (dt_log) dt_log[n_acc + n_rej] = h;
-            ++n_acc;
-            const double sug = cudisc_controller_next_dt(E, h);
-            dt = cut ? std::max(sug, dt) : sug;         // a step cut to land on t_span does not shrink dt
-        } else {                                        // reject: state and FSAL buffer untouched
-            if (dt_log) dt_log[n_acc + n_rej] = -h;
-            ++n_rej;
-            dt = cudisc_controller_next_dt(E, h);
-        }
-    }
-    if (cur != rho_dust) {
-        e = cudaMemcpyAsync(rho_dust, cur, row_bytes, cudaMemcpyDeviceToDevice, st);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        if (e != cudaSuccess) return cuda_fail(e, "integrate copy-back");
-    }
-    if (info) {
-        info->t_done = t; info->dt_last = dt_last; info->dt_next = dt; info->err_last = err_last;
-        info->n_accepted = n_acc; info->n_rejected = n_rej;
-    }
-    return status;
+    return integrate_impl(g, b, rho_dust, t_span, 0x7fffffff, dt_try, max_steps, dt_log, info, stream);
+}
+
+int cudisc_coag_integrate_steps(cudisc_grid g, cudisc_bins b, double *rho_dust, int n_accepted, double dt_try,
+                                int max_steps, double *dt_log, cudisc_integrate_info *info, cudisc_stream stream)
+{
+    int rc = check_pair(g, b);
+    if (rc) return rc;
+    if (!g->gas_bound) return fail(CUDISC_ERR_INVALID, "no gas state bound (cudisc_grid_bind_gas)");
+    if (!rho_dust) return fail(CUDISC_ERR_INVALID, "NULL array argument");
+    if (n_accepted < 1 || !(dt_try > 0.0) || max_steps < n_accepted)
+        return fail(CUDISC_ERR_INVALID, "need n_accepted >= 1, dt_try > 0, max_steps >= n_accepted");
+    return integrate_impl(g, b, rho_dust, 1.0e300, n_accepted, dt_try, max_steps, dt_log, info, stream);
 }
 
 int cudisc_microbench_dfma(int n_iter, double *dfma_per_s, double *elapsed_ms)

@@ -462,8 +462,10 @@ __device__ __forceinline__ double fast_eval(const DevTables &tb, const FastTable
 
 template <int NT, int MODE>
 __global__ void __launch_bounds__(NT, 1)
-coag_fast_kernel(const DevTables tb, const FastTables ft, const GasArgs gs, const StepArgs sa)
+coag_fast_kernel(const DevTables tb, const FastTables ft, const GasArgs gs, const StepArgs sa_in)
 {
+    StepArgs sa = sa_in;
+    if (MODE == MODE_STEP && !apply_ctrl(sa)) return;
     extern __shared__ __align__(16) double smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
     const int N = tb.N, Np = tb.Np;

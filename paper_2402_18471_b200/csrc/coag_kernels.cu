@@ -386,8 +386,10 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
 
 template <int NT, int MODE, bool SLAB, bool VINT>
 __global__ void __launch_bounds__(NT, 1)
-coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa)
+coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
 {
+    StepArgs sa = sa_in;
+    if ((MODE == MODE_STEP || MODE == MODE_STEPK) && !apply_ctrl(sa)) return;
     extern __shared__ __align__(16) double smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int N = tb.N, P = tb.P;
@@ -701,6 +703,54 @@ __global__ void __launch_bounds__(1024) err_max_kernel(const double *__restrict_
     for (int q = threadIdx.x; q < n; q += 1024) v = nanmax(v, err[q]);
     v = block_nanmax<1024>(v, red, threadIdx.x);   // 32 warps -> 32 slots
     if (threadIdx.x == 0) out[0] = v;
+}
+
+// Controller step (R10): E = max_c E_c; accept iff E <= 1; next size h clamp(0.9 E^(-1/3), 0.2, 5)
+// (5 for E == 0); the last step is cut to land on t_span and a cut step does not shrink the next size.
+__global__ void __launch_bounds__(1024) ctrl_kernel(const double *__restrict__ err, int n, CtrlState *cs,
+                                                    double *log)
+{
+    __shared__ double red[64];
+    if (cs->done) return;
+    double v = 0.0;
+    for (int q = threadIdx.x; q < n; q += 1024) v = nanmax(v, err[q]);
+    v = block_nanmax<1024>(v, red, threadIdx.x);
+    if (threadIdx.x != 0) return;
+    CtrlState c = *cs;
+    const double E = v, h = c.h;
+    const int slot = c.n_acc + c.n_rej;
+    if (!(E == E) || isinf(E)) {
+        c.status = 1; c.done = 1;
+        *cs = c;
+        return;
+    }
+    double f = 5.0;
+    if (E > 0.0) f = 0.9 * pow(E, -1.0 / 3.0);
+    f = fmin(5.0, fmax(0.2, f));
+    const double sug = h * f;
+    if (E <= 1.0) {
+        c.cur ^= 1; c.have_k1 = 1;
+        c.t = c.cut ? c.t_span : c.t + h;
+        c.dt_last = h; c.err_last = E;
+        if (log) log[slot] = h;
+        c.n_acc++;
+        c.dt = c.cut ? fmax(sug, c.dt) : sug;
+    } else {
+        if (log) log[slot] = -h;
+        c.n_rej++;
+        c.dt = sug;
+    }
+    if (c.t >= c.t_span || c.n_acc >= c.max_acc || c.n_acc + c.n_rej >= c.max_steps) c.done = 1;
+    const double left = c.t_span - c.t;
+    c.cut = c.dt >= left;
+    c.h = c.cut ? left : c.dt;
+    *cs = c;
+}
+
+cudaError_t launch_ctrl(const double *err, int n, CtrlState *cs, double *log, cudaStream_t st)
+{
+    ctrl_kernel<<<1, 1024, 0, st>>>(err, n, cs, log);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_err_max(const double *err, int n, double *out, cudaStream_t st)

@@ -26,6 +26,8 @@ cudaError_t launch_fast(int mode, const LaunchCfg &lc, const DevTables &tb, cons
 int cells_occupancy(int smem_bytes, int smem_optin);
 cudaError_t launch_dfma_peak(int grid, int n_iter, double *out, cudaStream_t st);
 cudaError_t launch_copy_peak(int grid, const void *src, void *dst, size_t n16, cudaStream_t st);
+// one controller update after a trial step (ctrl_kernel, coag_kernels.cu); log may be NULL
+cudaError_t launch_ctrl(const double *err, int n, CtrlState *cs, double *log, cudaStream_t st);
 // out[0] = NaN-propagating max of err[0..n)
 cudaError_t launch_err_max(const double *err, int n, double *out, cudaStream_t st);
 

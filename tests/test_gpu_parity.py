@@ -403,3 +403,29 @@ def test_empty_cell_among_populated_ones():
     info, log = cd.cudisc_coag_integrate(g.grid, g.bins, rho2, 3.0 * dt, dt, max_steps=100)
     torch.cuda.synchronize()
     assert info["t_done"] == 3.0 * dt and np.all(rho2.cpu().numpy()[2] == 0.0)
+
+
+def test_step_host_sliced_pipeline_is_bit_identical_to_device_step():
+    """Enough cells for the sliced end-to-end path (four slices on two internal streams): same bits as the
+    device-resident call, FSAL derivative carried across calls, sampled cells against the oracle."""
+    import torch
+    cfg, d = _disc(2, 5000)
+    po, pc = params_pair(cfg)
+    g = GpuDisc(d, pc)
+    dt = dt_of(2)
+    a = torch.from_numpy(d.rho_dust.copy()).pin_memory()
+    e = torch.empty(d.n_cells, dtype=torch.float64).pin_memory()
+    g2 = GpuDisc(d, pc)
+    b = g2.rho.clone()
+    for s in range(3):
+        cd.cudisc_coag_step_host(g.grid, g.bins, a, dt, e)
+        eb = g2.step(b, dt)
+        assert np.array_equal(a.numpy(), b.cpu().numpy()) and np.array_equal(e.numpy(), eb.cpu().numpy()), s
+    C = d.n_cells
+    cells = np.unique(np.array([0, 1, C // 4 - 1, C // 4, C // 2 - 1, C // 2, 3 * C // 4 - 1, 3 * C // 4, C - 1]))   # slice boundaries
+    ds = d.subset(cells)
+    r, k = ds.rho_dust.copy(), None
+    for s in range(3):
+        r, k, err_ref = orc.step_cells(*oracle_args(ds), po, r, dt, k1=k)
+    assert_rho_close(a.numpy()[cells], r, 3 * TOL_RHO_1, "sliced step_host, sampled cells")
+    np.testing.assert_allclose(e.numpy()[cells], err_ref, rtol=1e-6, atol=1e-12)
