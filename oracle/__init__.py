@@ -20,6 +20,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "coag_oracle.c"
+_SRC2 = _HERE / "hydro_oracle.c"
 _LIB = _HERE / "_build" / "liboracle.so"
 _lock = threading.Lock()
 _lib = None
@@ -51,11 +52,11 @@ class Params:
 def build(force: bool = False) -> Path:
     """Compile the oracle with gcc.  Building the checker is not using it."""
     with _lock:
-        if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        if force or not _LIB.exists() or _LIB.stat().st_mtime < max(_SRC.stat().st_mtime, _SRC2.stat().st_mtime):
             _LIB.parent.mkdir(exist_ok=True)
             tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
             cmd = ["gcc", "-O2", "-std=gnu11", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-                   "-o", str(tmp), str(_SRC), "-lm"]
+                   "-o", str(tmp), str(_SRC), str(_SRC2), "-lm"]
             subprocess.run(cmd, check=True)
             os.replace(tmp, _LIB)
     return _LIB
@@ -347,3 +348,15 @@ def replay(step, rho, dts):
     for h in dts:
         rho, k1, _ = step(rho, float(h), k1)
     return rho
+
+
+# ------------------------------------------------------------------------------------------ hydrostatic equilibrium
+def hydrostatic(R_e, tan_e, R_c, tan_c, cs2, Sigma, GM: float) -> np.ndarray:
+    """Gas density [n_r, n_z] of the vertical hydrostatic solve (Eqs. 32-37)."""
+    R_e = _in(R_e); tan_e = _in(tan_e); R_c = _in(R_c); tan_c = _in(tan_c); cs2 = _in(cs2); Sigma = _in(Sigma)
+    n_r, n_z = cs2.shape
+    assert R_e.size == n_r + 1 and tan_e.size == n_z + 1 and R_c.size == n_r and tan_c.size == n_z and Sigma.size == n_r
+    out = np.empty((n_r, n_z))
+    lib().orc_hydrostatic(C.c_int(n_r), C.c_int(n_z), _p(R_e), _p(tan_e), _p(R_c), _p(tan_c), _p(cs2), _p(Sigma),
+                          C.c_double(GM), _p(out))
+    return out
