@@ -345,6 +345,55 @@ def measured_peaks():
         return {}
 
 
+def run_hydro(args, dev):
+    """--entry hydro: cudisc_hydrostatic (Eqs. 32-37) on a grid large enough to leave the L2
+    (4096 x 1024 cells: 32 MiB read + 32 MiB written per launch); HBM-bound, 16 B per cell."""
+    import torch
+
+    import paper_2402_18471_b200 as cd
+    from paper_2402_18471_b200 import synth_disc as sd
+    n_r, n_z = 4096, 1024
+    R_e = 1.0 * sd.AU * 200.0 ** (np.arange(n_r + 1) / n_r)
+    R_c = np.sqrt(R_e[:-1] * R_e[1:])
+    tan_e = 0.3 * np.arange(n_z + 1) / n_z
+    tan_c = 0.5 * (tan_e[:-1] + tan_e[1:])
+    T = 150.0 * (R_c[:, None] / sd.AU) ** -0.5 * (1.0 + 3.0 * (tan_c[None, :] / 0.3) ** 2)
+    cs2 = torch.from_numpy(np.ascontiguousarray(sd.K_B * T / (2.4 * sd.M_H))).to(dev)
+    Sigma = torch.from_numpy(1000.0 * (R_c / sd.AU) ** -1.0).to(dev)
+    out = torch.empty_like(cs2)
+    h = cd.Hydro(R_e, tan_e, R_c, tan_c)
+    GM = sd.G_GRAV * sd.M_SUN
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    copy_bps, _ = cd.cudisc_microbench_copy(1 << 30)
+    peaks = measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs") or copy_bps / 1e9)
+    n0 = cd.cudisc_launch_count()
+    for _ in range(args.warmup):
+        cd.cudisc_hydrostatic(h, cs2, Sigma, GM, out)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    for e0, e1 in ev:
+        flush.zero_()
+        e0.record(stream)
+        cd.cudisc_hydrostatic(h, cs2, Sigma, GM, out)
+        e1.record(stream)
+    torch.cuda.synchronize()
+    sec = statistics.mean(e0.elapsed_time(e1) for e0, e1 in ev) * 1e-3
+    gbs = 16.0 * n_r * n_z / sec / 1e9
+    print(json.dumps({"entry": "hydro", "metric": "hydrostatic-equilibrium cells/s (cudisc_hydrostatic)",
+                      "value": n_r * n_z / sec, "unit": "cells/s", "ms_per_launch": 1e3 * sec, "dtype": "f64",
+                      "data": "synthetic", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+                      "config": {"workload": f"{n_r} x {n_z} cells, warm-surface temperature structure",
+                                 "l2": "flushed between timed launches"},
+                      "gpu_launches": int(cd.cudisc_launch_count() - n0),
+                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+                                   "frac": gbs / hbm_peak, "traffic": None,
+                                   "how": "16 B per cell (c_s^2 read, rho_g written) / mean CUDA-event launch duration",
+                                   "hbm_copy_measured_gbs": copy_bps / 1e9}}), flush=True)
+    return 0
+
+
 def run_entry(args):
     """--entry kernel | rates | step_cached | integrate: the other C-ABI entry points on the same workload
     (config 4 by default), each against its own roof: FP64 issue slots for `kernel`, HBM
@@ -359,6 +408,8 @@ def run_entry(args):
         raise RuntimeError("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
     dev = torch.device("cuda", env_int("LOCAL_RANK", 0))
     torch.cuda.set_device(dev)
+    if args.entry == "hydro":
+        return run_hydro(args, dev)
     cfg = synth_disc.CONFIGS[args.config]
     full = args.entry == "integrate"
     n_cells = cfg.n_cells if full else min(cfg.n_cells, args.cells)
@@ -475,7 +526,7 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--entry", choices=["step", "kernel", "rates", "step_cached", "integrate"], default="step",
+    ap.add_argument("--entry", choices=["step", "kernel", "rates", "step_cached", "integrate", "hydro"], default="step",
                     help="C-ABI entry point to time (default: cudisc_coag_step, the contract line)")
     ap.add_argument("--cells", type=int, default=16000, help="cells of the workload for --entry kernel/rates/step_cached")
     ap.add_argument("--accepted", type=int, default=1000, help="accepted steps of --entry integrate")

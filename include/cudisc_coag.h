@@ -254,6 +254,33 @@ int cudisc_coag_integrate_steps(cudisc_grid g, cudisc_bins b, double *rho_dust, 
                                 cudisc_stream stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Vertical hydrostatic equilibrium of the gas (Eqs. 32-37): the step
+ * that produces the rho_gas the coagulation path consumes.
+ * ------------------------------------------------------------------------------------------- */
+
+typedef struct cudisc_hydro_s *cudisc_hydro;   /* grid geometry on the device; owned by the library */
+
+/* Geometry of the (R, theta) grid of PAPER.md:29-38: R_edges [n_r + 1], tan_edges [n_z + 1] (tan theta at
+ * the cell interfaces, j = 0 nearest the mid-plane), R_centres [n_r], tan_centres [n_z] (HOST, copied;
+ * strictly increasing, centres inside their cells).  Uploads d(R^3)_i (Eq. 1), (R dR)_i = d(R^2)_i / 2
+ * (PAPER.md:264), d(tan theta)_j and the centres to the current device.  n_z <= 4096. */
+int cudisc_hydro_create(int n_r, int n_z, const double *R_edges, const double *tan_edges,
+                        const double *R_centres, const double *tan_centres, cudisc_hydro *out);
+int cudisc_hydro_destroy(cudisc_hydro h);
+
+/* rho_gas_out [n_r x n_z] (DEVICE, j fastest) <- hydrostatic gas density of every radial column:
+ *   P_{i,j} / P_{i,j-1} = exp[ GM <1/c_s^2>_{i,j} (1/r_{i,j} - 1/r_{i,j-1}) ]   (Eqs. 34, 35),
+ *   r_{i,j} = R^c_i sqrt(1 + tan^2 theta^c_j); multiplicative scan over j from the cell nearest the
+ *   mid-plane (Eq. 36; reading R17); omega = P / c_s^2; rho = Sigma_g (R dR) omega / sum_k omega V (Eq. 37,
+ *   taken literally: the cells on the grid carry Sigma_g, reading R18).
+ * cs2: DEVICE [n_r x n_z] isothermal sound speed squared, cm^2/s^2 (k_B T / mu m_H); Sigma_g: DEVICE [n_r],
+ * g/cm^2; GM: G M_*, cm^3/s^2.  May not alias.  Only enqueues on `stream`; allocates nothing. */
+int cudisc_hydrostatic(cudisc_hydro h, const double *cs2, const double *Sigma_g, double GM,
+                       double *rho_gas_out, cudisc_stream stream);
+
+const char *cudisc_hydro_last_error(void);
+
+/* ---------------------------------------------------------------------------------------------
  * Roofline denominators measured in the same process (north_star: "peaks measured by a
  * microbenchmark in the same run").  Both synchronise the device.
  * ------------------------------------------------------------------------------------------- */

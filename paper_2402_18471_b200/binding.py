@@ -48,6 +48,7 @@ EXPORTS = [
     "cudisc_coag_step", "cudisc_coag_step_cached", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_coag_integrate_steps", "cudisc_controller_next_dt",
     "cudisc_microbench_dfma",
     "cudisc_microbench_copy", "cudisc_launch_count", "cudisc_last_error", "cudisc_version",
+    "cudisc_hydro_create", "cudisc_hydro_destroy", "cudisc_hydrostatic", "cudisc_hydro_last_error",
 ]
 
 _lib = None
@@ -88,6 +89,10 @@ def lib() -> C.CDLL:
         L.cudisc_microbench_dfma.argtypes = [C.c_int, dp, dp]
         L.cudisc_microbench_copy.argtypes = [C.c_longlong, dp, dp]
         L.cudisc_launch_count.restype = C.c_longlong
+        L.cudisc_hydro_create.argtypes = [C.c_int, C.c_int, dp, dp, dp, dp, C.POINTER(vp)]
+        L.cudisc_hydro_destroy.argtypes = [vp]
+        L.cudisc_hydrostatic.argtypes = [vp, vp, vp, C.c_double, vp, vp]
+        L.cudisc_hydro_last_error.restype = C.c_char_p
         L.cudisc_last_error.restype = C.c_char_p
         L.cudisc_version.restype = C.c_char_p
         for name in EXPORTS:
@@ -342,6 +347,45 @@ def cudisc_coag_integrate_steps(grid: Grid, bins: Bins, rho_dust, n_accepted: in
                                              log.ctypes.data_as(C.POINTER(C.c_double)), C.byref(info),
                                              _stream(stream)))
     return _info_dict(info, log)
+
+
+class Hydro:
+    """cudisc_hydro handle: geometry of the (R, theta) grid for cudisc_hydrostatic."""
+
+    def __init__(self, R_edges, tan_edges, R_centres, tan_centres):
+        dp = C.POINTER(C.c_double)
+        a = [np.ascontiguousarray(x, dtype=np.float64) for x in (R_edges, tan_edges, R_centres, tan_centres)]
+        self.n_r, self.n_z = a[2].size, a[3].size
+        if a[0].size != self.n_r + 1 or a[1].size != self.n_z + 1:
+            raise ValueError("edge arrays must have one more entry than the centre arrays")
+        self._h = C.c_void_p()
+        code = lib().cudisc_hydro_create(self.n_r, self.n_z, *[x.ctypes.data_as(dp) for x in a], C.byref(self._h))
+        if code:
+            raise CudiscError(code, lib().cudisc_hydro_last_error().decode())
+
+    @property
+    def handle(self):
+        return self._h
+
+    def close(self):
+        if self._h:
+            lib().cudisc_hydro_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def cudisc_hydrostatic(hydro: Hydro, cs2, Sigma_g, GM: float, rho_gas_out, stream=None) -> None:
+    """rho_gas_out [n_r, n_z] <- vertical hydrostatic equilibrium of every column (Eqs. 32-37)."""
+    n = hydro.n_r * hydro.n_z
+    code = lib().cudisc_hydrostatic(hydro.handle, _dev_ptr(cs2, "cs2", n), _dev_ptr(Sigma_g, "Sigma_g", hydro.n_r),
+                                    float(GM), _dev_ptr(rho_gas_out, "rho_gas_out", n), _stream(stream))
+    if code:
+        raise CudiscError(code, lib().cudisc_hydro_last_error().decode())
 
 
 def cudisc_microbench_dfma(n_iter: int = 0):

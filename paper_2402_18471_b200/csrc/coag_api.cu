@@ -1461,6 +1461,8 @@ int cudisc_microbench_copy(long long n_bytes, double *bytes_per_s, double *elaps
 }
 
 long long cudisc_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+/* internal: the other translation units of the library report their launches here */
+void cudisc_count_launch_(void) { g_launches.fetch_add(1, std::memory_order_relaxed); }
 const char *cudisc_last_error(void) { return g_err; }
 const char *cudisc_version(void) { return "cudisc-coag-b200 0.1 (sm_100a)"; }
 
