@@ -227,3 +227,64 @@ def sample_cells(cfg: DiscConfig, n: int, seed: int = 7) -> np.ndarray:
     fixed = np.array([0, cfg.n_z - 1, C - cfg.n_z, C - 1, C // 2], dtype=np.int64)
     rest = rng.choice(C, size=max(n - fixed.size, 0), replace=False)
     return np.unique(np.concatenate([fixed, rest]))[:n]
+
+
+# ------------------------------------------------------------------------------------------ Fig. 10 set-up
+@dataclass
+class Fig10Inputs:
+    """Single-radius, vertically integrated coagulation test of PAPER.md:482-491 (Fig. 10): one cell per
+    alpha value at R = 20 AU.  rho_dust holds dust SURFACE densities (g/cm^2), h_dust the dust scale
+    heights, v_Z the terminal settling velocities at Z = h_i, rho_gas the mid-plane gas density."""
+    n_bins: int
+    a_min: float
+    a_max: float
+    rho_m: float
+    mu: float
+    v_frag: float
+    T: np.ndarray
+    rho_gas: np.ndarray
+    Omega: np.ndarray
+    alpha: np.ndarray
+    sigma_g: np.ndarray
+    c_s: np.ndarray
+    v_R: np.ndarray
+    v_Z: np.ndarray
+    h_dust: np.ndarray
+    rho_dust: np.ndarray
+    a_frag: np.ndarray      # (2 / 3 pi) Sigma_g / (rho_m alpha) (v_frag / c_s)^2, the fragmentation limit (PAPER.md:561)
+
+    @property
+    def n_cells(self) -> int:
+        return self.T.shape[0]
+
+
+def make_fig10(alphas=(1e-3, 1e-4), n_bins: int = 200, a_min: float = 1e-5, a_max: float = 10.0,
+               r_au: float = 20.0, T0: float = 36.0, mu: float = 2.4, v_frag: float = 100.0,
+               sigma0: float = 1000.0, rho_m: float = 1.67, dust_to_gas: float = 0.01) -> Fig10Inputs:
+    """PAPER.md:482-491 gives R = 20 AU, T = 36 K, mu = 2.4, alpha = 1e-3, v_frag = 100 cm/s, 200 species;
+    it does not give Sigma_g, the size range or the initial condition: Sigma_g = 1000 (R/AU)^-1 g/cm^2 (the
+    recipe of the five configs), 0.1 um - 10 cm, MRN up to 1 um with dust-to-gas 0.01 (R19).  A
+    second cell with alpha = 1e-4 moves the fragmentation limit by a factor 10 (scaling check)."""
+    alphas = np.asarray(alphas, dtype=np.float64)
+    C = alphas.size
+    R = r_au * AU
+    T = np.full(C, T0)
+    c_s = np.sqrt(K_B * T / (mu * M_H))
+    Om = np.full(C, np.sqrt(G_GRAV * M_SUN / R ** 3))
+    H = c_s / Om
+    sigma_g = np.full(C, sigma0 / r_au)
+    rho_mid = sigma_g / (np.sqrt(2.0 * np.pi) * H)
+    a_e, a_c = size_bins(n_bins, a_min, a_max)
+    St = 0.5 * np.pi * rho_m * a_c[None, :] / sigma_g[:, None]                 # mid-plane, Epstein
+    h = H[:, None] * np.sqrt(alphas[:, None] / (alphas[:, None] + St))         # PAPER.md:486
+    fac = St / (1.0 + St * St)
+    v_Z = -(Om[:, None] * h) * fac                                             # terminal settling at Z = h_i
+    v_k = np.sqrt(G_GRAV * M_SUN / R)
+    v_R = -2.0 * (0.5 * (c_s ** 2 / v_k) * 2.75)[:, None] * fac
+    w = _mrn_weights(a_e, 1e-4)
+    sig_d = dust_to_gas * sigma_g[:, None] * w[None, :]
+    a_frag = (2.0 / (3.0 * np.pi)) * sigma_g / (rho_m * alphas) * (v_frag / c_s) ** 2
+    return Fig10Inputs(n_bins=n_bins, a_min=a_min, a_max=a_max, rho_m=rho_m, mu=mu, v_frag=v_frag, T=T,
+                       rho_gas=rho_mid, Omega=Om, alpha=alphas, sigma_g=sigma_g, c_s=c_s,
+                       v_R=np.ascontiguousarray(v_R), v_Z=np.ascontiguousarray(v_Z),
+                       h_dust=np.ascontiguousarray(h), rho_dust=np.ascontiguousarray(sig_d), a_frag=a_frag)
