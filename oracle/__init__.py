@@ -140,6 +140,15 @@ def vrel2_turb(St1: float, St2: float, S: float, St_eta: float) -> float:
     return float(lib().orc_vrel2_turb(St1, St2, S, St_eta))
 
 
+VAR_NUMBER_SPLIT, VAR_TOTAL_LOOKUP = 1, 2
+
+
+def set_variant(v: int) -> None:
+    """Switches the two unpinned readings for the whole oracle (coag_oracle.c, orc_set_variant): bit 0 =
+    number-conserving two-bin split (G11), bit 1 = fragment l-bin looked up with the total fragment mass (G2)."""
+    lib().orc_set_variant(C.c_int(int(v)))
+
+
 def split(g: MassGrid, m: float):
     eps = C.c_double()
     l = lib().orc_split(C.c_int(g.N), _p(g.m_c), C.c_double(m), C.byref(eps))

@@ -188,6 +188,18 @@ void orc_vint_scale(int N, const double *hd, double *K)
  *   m <  m_0      -> l = -1, eps = 0   (all of it to bin 0)
  *   m >= m_{N-1}  -> l = N-1, eps = 1  (all of it to bin N-1)
  * ------------------------------------------------------------------------------------------ */
+/* Variants of two readings the paper cannot pin (R2, R11), switched for the
+ * whole oracle by orc_set_variant (default 0 = the readings taken):
+ *   bit 0 (ORC_VAR_NUMBER_SPLIT)  PAPER.md:446 "fractions of the mass": instead of the literal mass
+ *         fractions (eps m, (1 - eps) m) the two bins receive the NUMBER fractions eps, 1 - eps of the
+ *         product (Kovetz & Olund 1969): masses eps m_l and (1 - eps) m_u, which also sum to m.
+ *   bit 1 (ORC_VAR_TOTAL_LOOKUP)  PAPER.md:469-476: the l-bin of the largest fragment is looked up with
+ *         the total fragment mass m_j + min(chi m_j, m_i) instead of min(chi m_j, m_i). */
+enum { ORC_VAR_NUMBER_SPLIT = 1, ORC_VAR_TOTAL_LOOKUP = 2 };
+static int orc_variant = 0;
+void orc_set_variant(int v) { orc_variant = v; }
+int orc_get_variant(void) { return orc_variant; }
+
 int orc_split(int N, const double *m_c, double m, double *eps)
 {
     if (m < m_c[0]) { *eps = 0.0; return -1; }
@@ -195,6 +207,7 @@ int orc_split(int N, const double *m_c, double m, double *eps)
     int l = 0;
     while (l + 1 < N && m_c[l + 1] <= m) ++l;
     *eps = (m_c[l + 1] - m) / (m_c[l + 1] - m_c[l]);     /* Eq. 65 */
+    if (orc_variant & ORC_VAR_NUMBER_SPLIT) *eps = *eps * m_c[l] / m;   /* number eps -> mass eps m_l / m */
     return l;
 }
 
@@ -215,6 +228,7 @@ static void outcome_masses(double mi, double mj, double chi, double *m_rem, doub
     *m_rem = (x < mi) ? (mi - x) : 0.0;
     *m_lf = (x < mi) ? x : mi;
     *m_ft = mj + *m_lf;
+    if (orc_variant & ORC_VAR_TOTAL_LOOKUP) *m_lf = *m_ft;
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -334,8 +348,15 @@ void orc_rates_flux_cf(int N, const double *m_c, const double *m_e, const double
             /* --- coagulation product m_i + m_j (Eq. 63) */
             if (i < N - 1 && mj < m_c[i + 1] - mi) {
                 double D = m_c[i + 1] - mi;                              /* product inside [m_i, m_{i+1}) */
-                addpm(drho, g, l, i, Rc * mj * (m_c[i + 1] - 2.0 * mi - mj) / D);
-                addpm(drho, g, l, i + 1, Rc * mj * (mi + mj) / D);
+                if (orc_variant & ORC_VAR_NUMBER_SPLIT) {
+                    /* number eps = (D - m_j)/D stays in bin i (mass eps m_i, minus the m_i removed), number
+                       m_j / D arrives in bin i+1 with mass m_{i+1} each: -m_i m_j / D and + m_{i+1} m_j / D */
+                    addpm(drho, g, l, i, -Rc * mj * mi / D);
+                    addpm(drho, g, l, i + 1, Rc * mj * m_c[i + 1] / D);
+                } else {
+                    addpm(drho, g, l, i, Rc * mj * (m_c[i + 1] - 2.0 * mi - mj) / D);
+                    addpm(drho, g, l, i + 1, Rc * mj * (mi + mj) / D);
+                }
                 addpm(drho, g, l, j, -Rc * mj);
             } else if (i == N - 1) {                                     /* R8: stays in the top bin */
                 addpm(drho, g, l, N - 1, Rc * mj);
@@ -354,8 +375,14 @@ void orc_rates_flux_cf(int N, const double *m_c, const double *m_e, const double
             outcome_masses(mi, mj, chi, &m_rem, &m_ft, &m_lf);
             if (i >= 1 && chi * mj <= mi - m_c[i - 1]) {                 /* remnant inside (m_{i-1}, m_i] */
                 double Dp = mi - m_c[i - 1];
-                addpm(drho, g, l, i, -Rf * chi * mj * (1.0 + m_rem / Dp));
-                addpm(drho, g, l, i - 1, Rf * m_rem * chi * mj / Dp);
+                if (orc_variant & ORC_VAR_NUMBER_SPLIT) {
+                    /* number chi m_j / D' of the remnant drops to bin i-1 (mass m_{i-1} each) */
+                    addpm(drho, g, l, i, -Rf * chi * mj * mi / Dp);
+                    addpm(drho, g, l, i - 1, Rf * chi * mj * m_c[i - 1] / Dp);
+                } else {
+                    addpm(drho, g, l, i, -Rf * chi * mj * (1.0 + m_rem / Dp));
+                    addpm(drho, g, l, i - 1, Rf * m_rem * chi * mj / Dp);
+                }
                 addpm(drho, g, l, j, -Rf * mj);
             } else {
                 addpm(drho, g, l, i, -Rf * mi);

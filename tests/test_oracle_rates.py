@@ -18,7 +18,7 @@ import oracle as orc
 # ------------------------------------------------------------------------------------------
 # (a) the paper's definition in exact arithmetic
 # ------------------------------------------------------------------------------------------
-def literal_exact(m_c, m_e, K, pf, rho, eta_int, chi):
+def literal_exact(m_c, m_e, K, pf, rho, eta_int, chi, variant=0):
     """Eq. 53 with Eq. 54 (loss), Eq. 61 (gain), Eqs. 63-65 (C, R), Eq. 67 (F = N_k(m^e_{l+1})),
     Eq. 68 (m_rem), in Fractions.  eta_int: integer eta so that (.)^(2-eta) stays rational.
     Readings: R1 (1/2 on the diagonal in the gain only), R2, R5 (j <= i), R7, R8."""
@@ -44,6 +44,9 @@ def literal_exact(m_c, m_e, K, pf, rho, eta_int, chi):
             eps = (m[l + 1] - mass) / (m[l + 1] - m[l])       # Eq. 65
             w[l] = eps
             w[l + 1] = 1 - eps
+            if variant & 1:     # G11: eps is the NUMBER fraction; the mass fractions are eps m_l / m, (1 - eps) m_u / m
+                w[l] = eps * m[l] / mass
+                w[l + 1] = (1 - eps) * m[l + 1] / mass
         return w
 
     out = [Fr(0)] * N
@@ -56,9 +59,11 @@ def literal_exact(m_c, m_e, K, pf, rho, eta_int, chi):
             m_rem = m[i] - x if x < m[i] else Fr(0)            # Eq. 68
             m_ft = m[i] + m[j] - m_rem
             m_lf = min(x, m[i])
+            if variant & 2:     # G2: look the largest fragment's bin up with the total fragment mass
+                m_lf = m_ft
             Cw = split_weights(m[i] + m[j])
             Rw = split_weights(m_rem) if m_rem > 0 else [Fr(0)] * N
-            l = min(k for k in range(N) if me[k + 1] > m_lf)
+            l = min((k for k in range(N) if me[k + 1] > m_lf), default=N - 1)    # PAPER.md:469 (R8: clamped to the last bin)
             mmax = me[l + 1]
             Fw = [(me[k + 1] ** ex - me[k] ** ex) / (mmax ** ex - me[0] ** ex) if k <= l else Fr(0)
                   for k in range(N)]                            # Eq. 67
@@ -276,3 +281,53 @@ def test_cells_batch_matches_single_cell_and_planes_roundtrip():
         ds, gs, ls, _ = orc.rates_flux(g, K, pf, rho[c])
         assert np.array_equal(ds, d[c])
         assert np.array_equal(orc.pack_planes(K, pf), Kp[c])
+
+
+# ------------------------------------------------------------------------------------------
+# (e) the two switched readings (R2 / R11)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("q,chi", [(1.3, 1.0), (1.7, 0.5), (2.0, 2.0), (2.4, 1.0)])
+def test_variants_flux_form_equals_their_exact_definition_and_conserve_mass(variant, q, chi):
+    N = 8
+    try:
+        orc.set_variant(variant)
+        for eta_int, seed in ((1, 21), (0, 22)):
+            g, K, pf, rho = _random_problem(N, q, seed + int(q * 10))
+            exact = literal_exact(g.m_c, g.m_e, K, pf, rho, eta_int, chi, variant=variant)
+            assert sum(exact) == 0                                   # mass is conserved exactly by either reading
+            d, gain, loss, S = orc.rates_flux(g, K, pf, rho, eta=float(eta_int), chi=chi)
+            lit = orc.rates_literal(g, K, pf, rho, eta=float(eta_int), chi=chi)
+            scale = gain + loss
+            for k in range(N):
+                assert abs(d[k] - float(exact[k])) <= 2e-14 * scale[k]
+                assert abs(lit[k] - float(exact[k])) <= 2e-15 * scale[k] + 1e-300
+            # the variant is not the default reading
+            base = literal_exact(g.m_c, g.m_e, K, pf, rho, eta_int, chi, variant=0)
+            assert any(a != b for a, b in zip(exact, base))
+    finally:
+        orc.set_variant(0)
+
+
+def test_number_conserving_split_removes_exactly_one_particle_per_collision():
+    """G11 pin: with sticking only and every product on the grid, each collision turns two particles into one,
+    so d/dt sum_k n_k = - sum_{i >= j} R_ij EXACTLY for the number-weighted split -- and not for the
+    mass-weighted one (which creates or destroys particles when it splits a product over two bins)."""
+    N, q = 10, 1.6
+    g, K, pf, rho = _random_problem(N, q, 77)
+    pf[:] = 0.0
+    rho[N - 3:] = 0.0                                 # nothing can leave the top of the grid (q^3 > 2)
+    m = [Fr(x) for x in g.m_c]
+    n = [Fr(r) / mk for r, mk in zip(rho, m)]
+    collisions = sum(n[i] * n[j] * Fr(K[i][j]) * (Fr(1, 2) if i == j else 1) for i in range(N) for j in range(i + 1))
+    for variant, exact_number in ((1, True), (0, False)):
+        ex = literal_exact(g.m_c, g.m_e, K, pf, rho, 1, 1.0, variant=variant)
+        dN = sum(e / mk for e, mk in zip(ex, m))
+        assert (dN == -collisions) == exact_number
+        try:
+            orc.set_variant(variant)
+            d, gain, loss, _ = orc.rates_flux(g, K, pf, rho, eta=1.0, chi=1.0)
+        finally:
+            orc.set_variant(0)
+        dN_f = float(np.sum(d / g.m_c))
+        assert abs(dN_f - float(dN)) <= 1e-13 * float(collisions)
