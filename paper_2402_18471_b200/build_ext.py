@@ -13,8 +13,8 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libcudisc_coag.so"
-SOURCES = ["coag_api.cu", "coag_kernels.cu", "coag_fast.cu", "hydro.cu", "coag_tables.cpp"]
-HEADERS = ["coag_device.cuh", "coag_fast.h", "coag_launch.h", "coag_tables.h", "../../include/cudisc_coag.h"]
+SOURCES = ["coag_api.cu", "coag_kernels.cu", "coag_v3.cu", "coag_v3_host.cpp", "hydro.cu", "coag_tables.cpp"]
+HEADERS = ["coag_device.cuh", "coag_v3.h", "coag_launch.h", "coag_tables.h", "../../include/cudisc_coag.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=true"]
 

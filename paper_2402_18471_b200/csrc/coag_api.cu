@@ -13,7 +13,7 @@
 #include <string>
 #include <vector>
 
-#include "coag_fast.h"
+#include "coag_v3.h"
 #include "coag_launch.h"
 #include "coag_tables.h"
 
@@ -53,8 +53,7 @@ struct cudisc_bins_s {
     int device;
     void *dev_blob;
     DevTables dt;
-    FastTables ft;          // tensor-memory kernel tables (ft.on == 0: not applicable to this grid)
-    size_t fast_smem_bytes;
+    V3Tables v3;            // stencil cell kernel tables (v3.on == 0: not applicable to this grid)
 };
 
 struct cudisc_grid_s {
@@ -313,239 +312,6 @@ void build_schedule(const HostTables &t, Schedule &S)
     S.bini = std::move(bini);
 }
 
-// ---- schedule of the tensor-memory ("fast") kernel (coag_fast.h): static per-warp task lists.
-struct FastSchedule {
-    FastTables f;                       // scalars; pointers are set after the upload
-    std::vector<uint2> buildTasks, evalTasks;
-    std::vector<double> bandCoef;
-    std::vector<uint32_t> bandIdx;
-    size_t smemDoubles = 0;             // whole dynamic shared memory of the fast kernel, in doubles
-    std::string why;                    // reason the grid does not take the fast kernel (f.on == 0)
-};
-
-// cost model of the static schedule (cycles of one warp, measured on B200 with the phase counters of a
-// CUDISC_PROF build; only the ratios matter)
-constexpr long kCostBuildRow = 100, kCostBuildList32 = 130;
-constexpr long kCostRectCol = 60, kCostRagCol = 60, kCostTask = 100, kCostColTQuad = 180, kCostColSRow = 62, kCostW = 880;
-constexpr long kCostProloguePart = 1800;   // a third of the next cell's prologue, on the warps that own bins
-
-void build_fast_schedule(const HostTables &t, const Schedule &S, FastSchedule &F)
-{
-    const DevTables &d = S.d;
-    const int N = d.N, nblk = (N + 31) / 32, nWarps = kThreads / 32;
-    FastTables f;
-    memset(&f, 0, sizeof(f));
-    F.f = f;
-    F.buildTasks.clear(); F.evalTasks.clear(); F.bandCoef.clear(); F.bandIdx.clear();
-    if (!d.bandD || d.bandD > 8) { F.why = "band product stage does not fit"; return; }
-    if (N < 64) { F.why = "fewer than 64 bins"; return; }
-    const int nw = nblk;
-    if (2 * nw > nWarps || nblk > kFastMaxBlk) { F.why = "too many bins for the two combine groups"; return; }
-    f.nwBins = nw;
-
-    // ---- band tables in the padded target space: density group g <-> bins 32 g + lane, fragment-source
-    //      group g <-> l-bins 32 g + lane; stage index plane * bandD * Np + (i - j) * Np + i
-    std::vector<std::vector<std::pair<double, uint32_t>>> dens(N), frag(N);
-    for (const BandEntry &be : t.band) {          // sorted by (target, i, j, plane): fixed order
-        const uint32_t ix = (uint32_t)(be.plane * d.bandD * d.Np + (be.i - be.j) * d.Np + be.i);
-        if (be.i - be.j >= d.bandD) { F.why = "band entry outside the product stage"; return; }
-        (be.target < N ? dens[be.target] : frag[be.target - N]).push_back({be.coef, ix});
-    }
-    // table of entries [e0, e1) of every target of group g (e1 < 0: all), padded to a multiple of 4
-    auto emit_group = [&](const std::vector<std::vector<std::pair<double, uint32_t>>> &lists, int g, int part,
-                          int &len, int &off) {
-        int cmax = 0;
-        for (int k = 32 * g; k < std::min(N, 32 * g + 32); ++k) cmax = std::max(cmax, (int)lists[k].size());
-        const int cut = ((cmax + 1) / 2 + 3) & ~3;                 // first half: entries [0, cut)
-        const int e0 = part == 1 ? cut : 0, e1 = part == 0 ? cut : cmax;
-        len = std::max(4, (std::max(0, e1 - e0) + 3) & ~3);
-        off = (int)F.bandCoef.size();
-        F.bandCoef.resize(off + (size_t)len * 32, 0.0);
-        F.bandIdx.resize(off + (size_t)len * 32, 0u);
-        for (int k = 32 * g; k < std::min(N, 32 * g + 32); ++k)
-            for (int e = e0; e < std::min(e1, (int)lists[k].size()); ++e) {
-                F.bandCoef[off + (size_t)(e - e0) * 32 + (k & 31)] = lists[k][e].first;
-                F.bandIdx[off + (size_t)(e - e0) * 32 + (k & 31)] = lists[k][e].second;
-            }
-    };
-    for (int g = 0; g < nw; ++g) {
-        emit_group(dens, g, 0, f.bgLen[2 * g], f.bgOff[2 * g]);
-        emit_group(dens, g, 1, f.bgLen[2 * g + 1], f.bgOff[2 * g + 1]);
-        emit_group(frag, g, 2, f.sgLen[g], f.sgOff[g]);
-    }
-
-    // combine phase: warps < nw combine rows (light), warps [nw, 2 nw) combine columns, gather their own
-    // fragment-source group and scan (heavier); the density half-gathers go to the least loaded warps
-    int used[4];
-    for (int q = 0; q < 4; ++q) used[q] = fast_binc_cols(nw);
-    {
-        long load[kThreads / 32];
-        for (int w = 0; w < nWarps; ++w) load[w] = w < nw ? 150 : (w < 2 * nw ? 400 + 20L * f.sgLen[w - nw] : 0);
-        for (int g = 0; g < nw; ++g) {
-            f.sgCol[g] = used[(nw + g) & 3];
-            used[(nw + g) & 3] += 3 * f.sgLen[g];
-        }
-        int taken[kThreads / 32] = {0};
-        for (int gh = 0; gh < 2 * nw; ++gh) {
-            int best = -1;
-            for (int w = 0; w < nWarps; ++w)
-                if (taken[w] < 2 && (best < 0 || load[w] < load[best])) best = w;
-            taken[best]++;
-            f.bgWarp[gh] = best;
-            load[best] += 80 + 20L * f.bgLen[gh];
-            f.bgCol[gh] = used[best & 3];
-            used[best & 3] += 3 * f.bgLen[gh];
-        }
-    }
-    for (int q = 0; q < 4; ++q)
-        if (used[q] > kTmemCols) { F.why = "band tables exceed tensor memory"; return; }
-
-    // ---- column copy: quads (4 rows x 32 columns = 16 tensor-memory columns) of the rows i >= 32 c + 32
-    //      of column block c, walked in (c, row) order and dealt to the quarters in contiguous runs
-    struct Run { int q, c, r0, r1, tcol; };
-    std::vector<Run> runs, overflow;
-    {
-        int capQ[4], total = 0, capTotal = 0;
-        std::vector<int> quadsOf(nblk, 0);
-        for (int c = 0; c < nblk; ++c) {
-            quadsOf[c] = (std::max(0, N - (32 * c + 32)) + 3) / 4;
-            total += quadsOf[c];
-        }
-        for (int q = 0; q < 4; ++q) { capQ[q] = (kTmemCols - used[q]) / 16; capTotal += capQ[q]; }
-        int tgt[4] = {0, 0, 0, 0}, left = std::min(total, capTotal);
-        for (bool moved = true; left > 0 && moved;) {
-            moved = false;
-            int open = 0;
-            for (int q = 0; q < 4; ++q) open += tgt[q] < capQ[q];
-            if (!open) break;
-            const int share = std::max(1, left / open);
-            for (int q = 0; q < 4 && left > 0; ++q) {
-                const int give = std::min(std::min(share, capQ[q] - tgt[q]), left);
-                if (give > 0) { tgt[q] += give; left -= give; moved = true; }
-            }
-        }
-        int q = 0, fill = 0;
-        for (int c = 0; c < nblk; ++c) {
-            int r = 32 * c + 32, quads = quadsOf[c];
-            while (quads > 0) {
-                while (q < 4 && fill >= tgt[q]) { ++q; fill = 0; }
-                if (q >= 4) { overflow.push_back({4, c, r, N, kNoTmem}); break; }
-                const int n = std::min(quads, tgt[q] - fill);
-                runs.push_back({q, c, r, std::min(N, r + 4 * n), used[q] + 16 * fill});
-                fill += n; quads -= n; r += 4 * n;
-            }
-        }
-    }
-    f.colMask = 0;
-    for (const Run &ru : runs)
-        for (int j = 32 * ru.c; j < std::min(N, 32 * ru.c + 32); ++j)
-            if (t.iS[j] > ru.r0) f.colMask = 1;
-
-    // ---- tasks with costs and quarter constraints (quarter 4 = any warp)
-    struct Job { uint2 task; long cost; int q; };
-    std::vector<Job> bjobs, ejobs;
-    for (const Run &ru : runs)
-        for (int a = ru.r0; a < ru.r1; a += kFastRowsBuild) {
-            const int b = std::min(ru.r1, a + kFastRowsBuild);
-            bjobs.push_back({ftask_pack(FB_ROWS, ru.c, ru.tcol + 4 * (a - ru.r0), 0, a, b), kCostBuildRow * (b - a) + kCostTask, ru.q});
-        }
-    for (const Run &ru : overflow)
-        for (int a = ru.r0; a < ru.r1; a += kFastRowsBuild) {
-            const int b = std::min(ru.r1, a + kFastRowsBuild);
-            bjobs.push_back({ftask_pack(FB_ROWS, ru.c, kNoTmem, 0, a, b), kCostBuildRow * (b - a) + kCostTask, 4});
-        }
-    for (int c = 0; c < nblk; ++c) {
-        const int rows = std::min(32 * c + 32, N) - 32 * c;
-        const int last = rows * (rows + 1) / 2;
-        for (int a = 0; a < last; a += 96) {
-            const int b = std::min(last, a + 96);
-            bjobs.push_back({ftask_pack(FB_LIST, c, 0, 0, a, b), kCostBuildList32 * ((b - a + 31) / 32) + kCostTask, 4});
-        }
-    }
-
-    // column parts: contiguous per column block
-    {
-        std::vector<int> cnt(nblk, 0);
-        for (const Run &ru : runs) cnt[ru.c] += (ru.r1 - ru.r0 + kFastRowsColT - 1) / kFastRowsColT;
-        for (const Run &ru : overflow) cnt[ru.c] += (ru.r1 - ru.r0 + 31) / 32;
-        int base = 0;
-        for (int c = 0; c < nblk; ++c) { f.cpBase[c] = base; f.cpCnt[c] = cnt[c] + 1; base += cnt[c] + 1; }
-        f.nColParts = base;
-        std::vector<int> nextPart(nblk);
-        for (int c = 0; c < nblk; ++c) nextPart[c] = f.cpBase[c];
-        for (const Run &ru : runs)
-            for (int a = ru.r0; a < ru.r1; a += kFastRowsColT) {
-                const int b = std::min(ru.r1, a + kFastRowsColT);
-                ejobs.push_back({ftask_pack(FE_COLT, ru.c, ru.tcol + 4 * (a - ru.r0), nextPart[ru.c]++, a, b),
-                                 kCostColTQuad * ((b - a + 3) / 4) + kCostTask, ru.q});
-            }
-        for (const Run &ru : overflow)
-            for (int a = ru.r0; a < ru.r1; a += 32) {
-                const int b = std::min(ru.r1, a + 32);
-                ejobs.push_back({ftask_pack(FE_COLS, ru.c, 0, nextPart[ru.c]++, a, b), kCostColSRow * (b - a) + kCostTask, 4});
-            }
-        for (int c = 0; c < nblk; ++c)
-            ejobs.push_back({ftask_pack(FE_COLS, c, 0, nextPart[c]++, 32 * c, std::min(N, 32 * c + 32)),
-                             kCostColSRow * 32 + kCostTask, 4});
-    }
-    // row parts: per row block the rectangle [0, min n_bulk) in chunks, then the ragged rest
-    {
-        int base = 0;
-        for (int blk = 0; blk < nblk; ++blk) {
-            const int i0 = 32 * blk, i1 = std::min(N, i0 + 32);
-            int cmin = 1 << 30, cmax = 0;
-            for (int i = i0; i < i1; ++i) { cmin = std::min(cmin, t.n_bulk[i]); cmax = std::max(cmax, t.n_bulk[i]); }
-            cmin &= ~1;
-            f.rpBase[blk] = base;
-            int np = 0;
-            const int nch = (cmin + kFastRectCols - 1) / kFastRectCols;
-            for (int ch = 0; ch < nch; ++ch) {
-                // even split of the rectangle into nch chunks with even boundaries
-                const int a = ((long)cmin * ch / nch) & ~1, b = ch + 1 == nch ? cmin : (((long)cmin * (ch + 1) / nch) & ~1);
-                if (b > a) { ejobs.push_back({ftask_pack(FE_RECT, blk, 0, base + np, a, b), kCostRectCol * (b - a) + kCostTask, 4}); ++np; }
-            }
-            if (cmax > cmin) { ejobs.push_back({ftask_pack(FE_RAG, blk, 0, base + np, cmin, cmax), kCostRagCol * (cmax - cmin) + kCostTask, 4}); ++np; }
-            f.rpCnt[blk] = np;
-            base += np;
-        }
-        f.nRowParts = base;
-    }
-    for (int blk = 0; blk < nblk; ++blk) ejobs.push_back({ftask_pack(FE_W, blk, 0, 0, 0, 0), kCostW, 4});
-
-    // ---- longest-processing-time-first onto the warps (quarter-bound jobs first, then the free ones)
-    auto deal = [&](std::vector<Job> &jobs, std::vector<uint2> &out, int (&woff)[17], const long *preload) {
-        std::stable_sort(jobs.begin(), jobs.end(), [](const Job &x, const Job &y) {
-            if ((x.q < 4) != (y.q < 4)) return x.q < 4;
-            return x.cost > y.cost;
-        });
-        std::vector<std::vector<uint2>> lists(nWarps);
-        long load[kThreads / 32];
-        for (int w = 0; w < nWarps; ++w) load[w] = preload ? preload[w] : 0;
-        for (const Job &jb : jobs) {
-            int best = -1;
-            for (int w = 0; w < nWarps; ++w)
-                if ((jb.q == 4 || (w & 3) == jb.q) && (best < 0 || load[w] < load[best])) best = w;
-            lists[best].push_back(jb.task);
-            load[best] += jb.cost;
-        }
-        out.clear();
-        for (int w = 0; w < nWarps; ++w) {
-            woff[w] = (int)out.size();
-            out.insert(out.end(), lists[w].begin(), lists[w].end());
-        }
-        woff[nWarps] = (int)out.size();
-    };
-    long pre[kThreads / 32];
-    for (int w = 0; w < nWarps; ++w) pre[w] = w < nw ? kCostProloguePart : 0;
-    deal(bjobs, F.buildTasks, f.bw, nullptr);
-    deal(ejobs, F.evalTasks, f.ew, pre);
-
-    fast_layout(f, d.P, d.Np, d.bandD);
-    F.smemDoubles = (size_t)f.off[FO_END];
-    f.on = 1;
-    F.f = f;
-}
-
 int upload_tables(cudisc_bins b)
 {
     int dev = 0;
@@ -563,11 +329,13 @@ int upload_tables(cudisc_bins b)
     const std::vector<double> &binc = S.binc, &bcoef = S.bcoef, &dtab = S.dtab, &exptab = S.exptab;
     const std::vector<int2> &bini = S.bini;
 
-    FastSchedule F;
-    build_fast_schedule(t, S, F);
+    int optin = 0;
+    e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+    V3Host V;
+    v3_build(t, d.logGrid, optin, V);
     Blob bl;
-    const size_t o_fb = bl.add(F.buildTasks), o_fe = bl.add(F.evalTasks);
-    const size_t o_fbc = bl.add(F.bandCoef), o_fbi = bl.add(F.bandIdx);
+    const size_t o_vx = bl.add(V.exc);
     const size_t o_a = bl.add(t.a), o_binc = bl.add(binc), o_bini = bl.add(bini);
     const size_t o_cnt = bl.add(cnt), o_bidx = bl.add(bidx), o_bcoef = bl.add(bcoef);
     const size_t o_bI = bl.add(buildItems), o_eI = bl.add(evalItems);
@@ -587,10 +355,8 @@ int upload_tables(cudisc_bins b)
     d.dtab = (const double2 *)(base + o_dt); d.exptab = (const double *)(base + o_ex);
     d.sched = (const int *)(base + o_sc);
     b->dt = d;
-    b->ft = F.f;
-    b->ft.buildTasks = (const uint2 *)(base + o_fb); b->ft.evalTasks = (const uint2 *)(base + o_fe);
-    b->ft.bandCoef = (const double *)(base + o_fbc); b->ft.bandIdx = (const uint32_t *)(base + o_fbi);
-    b->fast_smem_bytes = F.smemDoubles * sizeof(double);
+    b->v3 = V.t;
+    b->v3.exc = (const V3Exc *)(base + o_vx);
     b->dev_blob = blob;
     b->device = dev;
     b->on_device = true;
@@ -647,9 +413,10 @@ int run(cudisc_grid g, int mode, GasArgs ga, StepArgs sa, cudisc_stream stream, 
     sa.prof = g->prof;
     LaunchCfg lc{std::min(g->grid_ctas, std::max(1, sa.C)), g->smem_bytes, g->smem_optin};
     cudaError_t e;
-    if (g->fast && (mode == MODE_OTF || mode == MODE_STEP) && !ga.hd) {
-        LaunchCfg lf{std::min(g->fast_ctas, std::max(1, sa.C)), (int)g->bins->fast_smem_bytes, g->smem_optin};
-        e = launch_fast(mode, lf, g->bins->dt, g->bins->ft, ga, sa, (cudaStream_t)stream);
+    if (g->fast && (mode == MODE_OTF || mode == MODE_STEP) && !ga.hd && !ga.vphi) {
+        LaunchCfg lf{std::min(g->fast_ctas, std::max(1, sa.C)), g->bins->v3.smemBytes, g->smem_optin};
+        sa.Psm = getenv("V3_DEBUG") ? atoi(getenv("V3_DEBUG")) : 0;
+        e = launch_v3(mode, lf, g->bins->dt, g->bins->v3, ga, sa, (cudaStream_t)stream);
     } else {
         e = launch_cells(mode, lc, g->bins->dt, ga, sa, (cudaStream_t)stream);
     }
@@ -851,112 +618,12 @@ int cudisc_bins_schedule_check(cudisc_bins b, long long *out)
             if (ntask < 1 || ntask > 2 || ent != Lg) ++bad[5];
         }
     }
-    // ---- the static schedule of the tensor-memory kernel, when this grid takes it (coag_fast.h): same
-    //      counters.  Tasks are decoded with ftask_unpack, the function the device uses.
-    FastSchedule F;
-    build_fast_schedule(t, S, F);
-    if (F.f.on) {
-        const FastTables &f = F.f;
-        const int nWarps = kThreads / 32;
-        std::vector<int> fbuilt((size_t)N * N, 0), frow((size_t)N * N, 0), fcol((size_t)N * N, 0);
-        // tensor-memory map: (quarter, column) -> row-slice id c * 4096 + i written by the build, read by COLT
-        std::vector<int> tmap(4 * kTmemCols, -1), tread(4 * kTmemCols, 0);
-        auto claim = [&](int q, int col, int n, int id) {        // band / per-bin constant regions
-            for (int u = col; u < col + n; ++u) {
-                if (u < 0 || u >= kTmemCols || tmap[q * kTmemCols + u] != -1) { ++bad[3]; continue; }
-                tmap[q * kTmemCols + u] = id;
-            }
-        };
-        for (int q = 0; q < 4; ++q) claim(q, 0, fast_binc_cols(f.nwBins), -2);
-        for (int gh = 0; gh < 2 * f.nwBins; ++gh) claim(f.bgWarp[gh] & 3, f.bgCol[gh], 3 * f.bgLen[gh], -3);
-        for (int g = 0; g < f.nwBins; ++g) claim((f.nwBins + g) & 3, f.sgCol[g], 3 * f.sgLen[g], -4);
-        for (int w = 0; w < nWarps; ++w)
-            for (int it = f.bw[w]; it < f.bw[w + 1]; ++it) {
-                const FTask k = ftask_unpack(F.buildTasks[it]);
-                if (k.kind == FB_ROWS) {
-                    for (int i = k.a; i < k.b; ++i)
-                        for (int lane = 0; lane < 32; ++lane) {
-                            const int j = 32 * k.blk + lane;
-                            if (j >= N) continue;
-                            if (i >= N || j >= i) { ++bad[0]; continue; }
-                            fbuilt[(size_t)i * N + j]++;
-                        }
-                    if (k.tcol != kNoTmem)
-                        for (int i = k.a; i < k.a + ((k.b - k.a + 1) & ~1); ++i) claim(w & 3, k.tcol + 4 * (i - k.a), 4, k.blk * 4096 + i);
-                } else {
-                    for (int tt = k.a; tt < k.b; ++tt) {
-                        int r = (int)((std::sqrt(8.0 * tt + 1.0) - 1.0) * 0.5);
-                        while (tri_h(r + 1) <= tt) ++r;
-                        while (tri_h(r) > tt) --r;
-                        const int i = 32 * k.blk + r, j = 32 * k.blk + (tt - tri_h(r));
-                        if (i >= N || j > i) { ++bad[0]; continue; }
-                        fbuilt[(size_t)i * N + j]++;
-                    }
-                }
-            }
-        std::vector<int> rpart(std::max(1, f.nRowParts), 0), cpart(std::max(1, f.nColParts), 0);
-        int nWtask = 0;
-        for (int w = 0; w < nWarps; ++w)
-            for (int it = f.ew[w]; it < f.ew[w + 1]; ++it) {
-                const FTask k = ftask_unpack(F.evalTasks[it]);
-                if (k.kind == FE_RECT || k.kind == FE_RAG) {
-                    if (k.slot < f.rpBase[k.blk] || k.slot >= f.rpBase[k.blk] + f.rpCnt[k.blk] || rpart[k.slot]++) ++bad[3];
-                    if (k.kind == FE_RECT && ((k.a | k.b) & 1)) ++bad[1];
-                    for (int i = 32 * k.blk; i < std::min(N, 32 * k.blk + 32); ++i)
-                        for (int j = k.a; j < k.b; ++j) {
-                            if (k.kind == FE_RECT && j >= t.n_bulk[i]) ++bad[1];      // the rectangle must be bulk
-                            if (j < t.n_bulk[i]) frow[(size_t)i * N + j]++;
-                        }
-                } else if (k.kind == FE_COLT || k.kind == FE_COLS) {
-                    if (k.slot < f.cpBase[k.blk] || k.slot >= f.cpBase[k.blk] + f.cpCnt[k.blk] || cpart[k.slot]++) ++bad[3];
-                    for (int i = k.a; i < k.b; ++i)
-                        for (int j = 32 * k.blk; j < std::min(N, 32 * k.blk + 32); ++j)
-                            if (i >= j) fcol[(size_t)i * N + j]++;
-                    if (k.kind == FE_COLT) {
-                        if (k.a < 32 * k.blk + 32 || (k.a & 1)) ++bad[2];
-                        for (int i = k.a; i < k.b; ++i) {
-                            const int u = (w & 3) * kTmemCols + k.tcol + 4 * (i - k.a);
-                            if (k.tcol + 4 * (i - k.a) + 4 > kTmemCols || tmap[u] != k.blk * 4096 + i) ++bad[3];
-                            else tread[u]++;
-                        }
-                        // the column copy masks Kf below iS[j]: only legal if the flag says so
-                        for (int j = 32 * k.blk; j < std::min(N, 32 * k.blk + 32); ++j)
-                            if (t.iS[j] > k.a && !f.colMask) ++bad[2];
-                    }
-                } else if (k.kind == FE_W) {
-                    ++nWtask;
-                } else ++bad[3];
-            }
-        for (int p = 0; p < f.nRowParts; ++p) bad[3] += rpart[p] != 1;
-        for (int p = 0; p < f.nColParts; ++p) bad[3] += cpart[p] != 1;
-        if (nWtask != (N + 31) / 32) ++bad[4];
-        for (int i = 0; i < N; ++i)
-            for (int j = 0; j <= i; ++j) {
-                bad[0] += fbuilt[(size_t)i * N + j] != 1;
-                bad[1] += frow[(size_t)i * N + j] != (j < t.n_bulk[i] ? 1 : 0);
-                bad[2] += fcol[(size_t)i * N + j] != 1;
-            }
-        // band tables: every entry of the host table exactly once, in order, with its stage index
-        long long fent = 0;
-        for (int gh = 0; gh < 2 * f.nwBins; ++gh)
-            for (int e = 0; e < f.bgLen[gh] * 32; ++e) fent += F.bandCoef[f.bgOff[gh] + e] != 0.0;
-        for (int g = 0; g < f.nwBins; ++g)
-            for (int e = 0; e < f.sgLen[g] * 32; ++e) fent += F.bandCoef[f.sgOff[g] + e] != 0.0;
-        long long nz = 0;
-        for (const BandEntry &be : t.band) nz += be.coef != 0.0;
-        if (fent != nz) ++bad[4];
-        for (uint32_t ix : F.bandIdx)
-            if (ix >= (uint32_t)(2 * d.bandD * Np)) ++bad[4];
-        int per[kThreads / 32] = {0};
-        for (int gh = 0; gh < 2 * f.nwBins; ++gh) {
-            if (f.bgWarp[gh] < 0 || f.bgWarp[gh] >= nWarps || ++per[f.bgWarp[gh]] > 2) ++bad[5];
-            if (f.bgLen[gh] & 3) ++bad[5];
-        }
-        if ((size_t)f.off[FO_END] != F.smemDoubles) ++bad[3];
-    }
+    // ---- the static run lists of the stencil cell kernel, when this grid takes it (coag_v3.h): same counters
+    V3Host V;
+    v3_build(t, d.logGrid, 232448, V);
+    if (V.t.on) v3_check(t, V, bad);
     for (int q = 0; q < 6; ++q) out[q] = bad[q];
-    out[6] = (long long)S.buildItems.size() + (long long)S.evalItems.size()
-             + (long long)F.buildTasks.size() + (long long)F.evalTasks.size();
+    out[6] = (long long)S.buildItems.size() + (long long)S.evalItems.size();
     out[7] = (long long)(smem_vec_doubles(Np, d.partRowSlots, d.partColSlots, d.nBuildItems + d.nEvalItems, d.bandD)
                          * sizeof(double));
     return CUDISC_OK;
@@ -967,19 +634,16 @@ int cudisc_bins_fast_path(cudisc_bins b, int *on, long long *smem_bytes, int *tm
     if (!bins_ok(b)) return fail(CUDISC_ERR_HANDLE, "bad bins handle");
     Schedule S;
     build_schedule(b->ht, S);
-    FastSchedule F;
-    build_fast_schedule(b->ht, S, F);
-    if (on) *on = F.f.on;
-    if (smem_bytes) *smem_bytes = F.f.on ? (long long)(F.smemDoubles * sizeof(double)) : 0;
+    V3Host V;
+    v3_build(b->ht, S.d.logGrid, 232448, V);
+    if (on) *on = V.t.on;
+    if (smem_bytes) *smem_bytes = V.t.on ? (long long)V.t.smemBytes : 0;
     if (tmem_cols_used) {
         int used = 0;
-        if (F.f.on) {
-            used = 4 * fast_binc_cols(F.f.nwBins);
-            for (int gh = 0; gh < 2 * F.f.nwBins; ++gh) used += 3 * F.f.bgLen[gh];
-            for (int g = 0; g < F.f.nwBins; ++g) used += 3 * F.f.sgLen[g];
-            for (uint2 u : F.buildTasks) {
-                const FTask k = ftask_unpack(u);
-                if (k.kind == FB_ROWS && k.tcol != kNoTmem) used += 4 * ((k.b - k.a + 1) & ~1);
+        if (V.t.on) {
+            for (int w = 0; w < kV3Warps; ++w) {
+                used += w < V.t.nb ? 16 : (w < 2 * V.t.nb ? 2 : 0);
+                for (int r = 0; r < kV3ColRuns; ++r) used += 32 * V.t.col[w][r].n;
             }
         }
         *tmem_cols_used = used;
@@ -1029,7 +693,7 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
     int per_sm = cells_occupancy(g->smem_bytes, optin);
     if (per_sm < 1) { delete g; return fail(CUDISC_ERR_CUDA, "kernel does not fit on an SM"); }
     g->grid_ctas = std::max(1, std::min(g->C, sms * per_sm));
-    g->fast = b->ft.on && b->fast_smem_bytes <= (size_t)optin && !getenv("CUDISC_NO_FAST");
+    g->fast = b->v3.on && b->v3.smemBytes <= optin && !getenv("CUDISC_NO_FAST");
     g->fast_ctas = std::max(1, std::min(g->C, sms));
 
     const size_t row_bytes = (size_t)g->C * d.N * sizeof(double);

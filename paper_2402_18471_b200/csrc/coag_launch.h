@@ -18,10 +18,10 @@ struct LaunchCfg {
 // mode: 0 kernel, 1 rates (supplied K), 2 rates on the fly, 3 BS3(2) step
 cudaError_t launch_cells(int mode, const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
                          const StepArgs &sa, cudaStream_t st);
-// the tensor-memory kernel (coag_fast.cu): MODE_OTF or MODE_STEP on a mass grid with ft.on
-struct FastTables;
-cudaError_t launch_fast(int mode, const LaunchCfg &lc, const DevTables &tb, const FastTables &ft,
-                        const GasArgs &gs, const StepArgs &sa, cudaStream_t st);
+// the stencil cell kernel (coag_v3.cu): MODE_OTF or MODE_STEP on a mass grid with vt.on
+struct V3Tables;
+cudaError_t launch_v3(int mode, const LaunchCfg &lc, const DevTables &tb, const V3Tables &vt,
+                      const GasArgs &gs, const StepArgs &sa, cudaStream_t st);
 // resident CTAs per SM of the cell kernels with `smem_bytes` of dynamic shared memory (0 on error)
 int cells_occupancy(int smem_bytes, int smem_optin);
 cudaError_t launch_dfma_peak(int grid, int n_iter, double *out, cudaStream_t st);

@@ -1,0 +1,707 @@
+// coag_v3.cu -- the stencil cell kernel (sm_100a, FP64): cudisc_coag_step and cudisc_coag_rates_otf on
+// mass grids that coag_v3_host.cpp accepts (every exact log grid whose cell fits an SM).
+//
+// Same mathematics and the same device routines (prologue, pair kernel, BS3(2) algebra) as the general
+// kernel of coag_kernels.cu; what differs is where the collision kernel of the cell lives and how the
+// work is dealt out (coag_v3.h):
+//   * the build writes every K_ij twice: to the packed shared-memory row copy and to the column copy in
+//     tensor memory (tcgen05.st, lane <-> column j, 8-row chunks); a 32 x 32 diagonal block is built with
+//     its short and long rows folded into full warps, then copied to tensor memory with zeros above the
+//     diagonal;
+//   * a rate evaluation reads the row copy once (row pass) and the column copy once (column pass, one
+//     tcgen05.ld.x32 per chunk, the next chunk in flight while the current one is summed);
+//   * the near-diagonal outcomes are a stencil over y_i n_{i-d} K[i][i-d] with warp-uniform coefficients
+//     from the constant bank (+ a few exception entries at the grid ends);
+//   * every warp owns a static list of runs (kernel parameter V3Tables): no queues, no atomics, fixed
+//     summation order -> results are bit-reproducible.
+// One persistent CTA of 512 threads per SM; thread k < N owns bin k (state and derivatives in registers).
+#include "coag_v3.h"
+#include "coag_launch.h"
+
+namespace cudisc {
+
+namespace {
+
+// ------------------------------------------------------------------------------------------ tensor memory
+__device__ __forceinline__ uint32_t tq_addr(uint32_t tbase, int quarter, int col)
+{
+    return tbase + ((uint32_t)(32 * quarter) << 16) + (uint32_t)col;
+}
+__device__ __forceinline__ void tmem_st2(uint32_t taddr, uint32_t a, uint32_t b)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};\n" :: "r"(taddr), "r"(a), "r"(b) : "memory");
+}
+__device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t (&v)[2])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];\n"
+                 : "=r"(v[0]), "=r"(v[1]) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+                 "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+                 "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};\n"
+                 :: "r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+                    "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
+                    "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
+                    "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                 "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                   "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                   "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                 : "r"(taddr) : "memory");
+}
+// 8-byte asynchronous global -> shared copy (LDGSTS): inputs of a cell are staged in shared memory
+// while the build runs, without holding registers across it
+__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src_gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n"
+                 :: "r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+__device__ __forceinline__ double u2d(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
+__device__ __forceinline__ uint32_t dlo(double x) { return (uint32_t)__double2loint(x); }
+__device__ __forceinline__ uint32_t dhi(double x) { return (uint32_t)__double2hiint(x); }
+__device__ __forceinline__ void named_barrier(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;\n" :: "r"(id), "r"(nthreads) : "memory");
+}
+
+// per-bin constants of the combine step in tensor memory (bin-owning warps: 8 doubles in 16 columns)
+enum { VB_A1 = 0, VB_A2, VB_B1, VB_F1, VB_F2, VB_G1, VB_FA, VB_PAD, kVBinc };
+
+// ------------------------------------------------------------------------------------------ shared memory
+struct VSm {
+    double2 *KR;        // row copy of the kernel, packed lower-triangular, diagonal halved
+    double2 *YY;        // (y, y m), index -kV3Pad .. Np + kV3Pad - 1 (zeros outside the bins)
+    double *NN;         // n = y / m, same padding
+    double *RED, *BAND, *GK, *SUF;
+    int2 *BINI;
+    double2 *COLP;      // [slot][32] (G, H) partial column sums
+    double2 *ROWP;      // [slot][32][2] (A1, A2), (F1, F2) partial row sums
+    Smem s;             // the arrays the shared device routines address (coag_device.cuh)
+};
+
+__device__ __forceinline__ VSm v3_carve(char *base, const V3Tables &vt)
+{
+    const int Np = 32 * vt.nb;
+    VSm f;
+    f.KR = (double2 *)(base + vt.oK);
+    f.YY = (double2 *)(base + vt.oYY) + kV3Pad;
+    f.NN = (double *)(base + vt.oNN) + kV3Pad;
+    f.RED = (double *)(base + vt.oRED);
+    f.BAND = (double *)(base + vt.oBAND);
+    f.GK = (double *)(base + vt.oGK);
+    f.SUF = f.GK + Np;
+    f.BINI = (int2 *)(base + vt.oNBULK);
+    f.COLP = (double2 *)(base + vt.oCOLP);
+    f.ROWP = (double2 *)(base + vt.oROWP);
+    Smem &s = f.s;
+    double *u = (double *)(base + vt.oUNION);
+    s.YY = f.YY; s.NN = f.NN;
+    s.DTAB = (double2 *)(base + vt.oDTAB);
+    s.EXPT = (double *)(base + vt.oEXPT);
+    s.RED = f.RED;
+    s.BANDV = s.BANDV2 = nullptr; s.WST = nullptr; s.BINC = nullptr; s.BINI = f.BINI;
+    s.CTR = nullptr; s.SCHED = nullptr; s.ITB = s.ITE = nullptr; s.PARTR = s.PARTC = nullptr;
+    s.RI = (double2 *)u;
+    s.B0 = (double2 *)(u + 10 * Np); s.B1 = (double2 *)(u + 12 * Np);
+    s.J2 = (double2 *)(u + 14 * Np); s.J3 = (double2 *)(u + 16 * Np);
+    s.V5 = u + 18 * Np;
+    return f;
+}
+
+// ------------------------------------------------------------------------------------------ build
+// rows [32 c + 8 k0, ...) of column block c in chunks of 8 rows (all rows >= 32 c + 32: no diagonal pair);
+// lanes <-> columns j = 32 c + lane.  Two rows per iteration.
+__device__ __forceinline__ void v3_build_rows(const V3Tables &vt, const VSm &f, const PairConst &pc,
+                                              const V3ColRun &run, uint32_t tq, int lane)
+{
+    const Smem &s = f.s;
+    const int N = vt.N;
+    const int j = 32 * run.c + lane;                 // < N: the block has rows below it
+    const RoleJ B = load_role_j<false>(s, j);
+    const int iSj = (f.BINI[j].x >> 9) & 0x1ff;
+    int i = 32 * run.c + 8 * run.k0;
+    const int iend = min(N, i + 8 * run.n);
+    uint32_t ta = tq + (uint32_t)run.tcol;
+    double2 *kr = f.KR + tri(i) + j;
+#pragma unroll 1
+    for (; i < iend; i += 2, ta += 8) {
+        const bool two = i + 1 < iend;
+        const int i2 = two ? i + 1 : i;
+        const RoleI A1 = load_role_i<false, false>(s, i);
+        const RoleI A2 = load_role_i<false, false>(s, i2);
+        const double2 k1 = pair_kernel<false, true, false>(A1, B, i - j, pc, s);
+        double2 k2 = pair_kernel<false, true, false>(A2, B, i2 - j, pc, s);
+        kr[0] = k1;
+        if (two) kr[i + 1] = k2;
+        else k2 = make_double2(0.0, 0.0);            // the row past the grid stays 0 in the column copy
+        kr += 2 * i + 3;                             // tri(i + 2) - tri(i)
+        // column copy: Kf of rows below iS[j] is not part of the column sums (coag_tables.h)
+        const double f1 = (i < iSj) ? 0.0 : k1.y, f2 = (i2 < iSj) ? 0.0 : k2.y;
+        const uint32_t v[8] = {dlo(k1.x), dhi(k1.x), dlo(f1), dhi(f1), dlo(k2.x), dhi(k2.x), dlo(f2), dhi(f2)};
+        tmem_st8(ta, v);
+    }
+}
+
+// diagonal block c: rows folded two to a warp (V3Tables::foldA / foldB), two folded rows per iteration;
+// then the block goes to tensor memory with zeros above the diagonal.
+__device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, const PairConst &pc,
+                                              const V3ColRun &run, uint32_t tq, int lane)
+{
+    const Smem &s = f.s;
+    const int N = vt.N, c = run.c, nf = vt.nFold[c];
+    auto where = [&](int fi, int &i, int &j) -> bool {
+        const int rA = vt.foldA[c][fi], rB = vt.foldB[c][fi];
+        bool ok = true;
+        int r = rA, q = lane;
+        if (lane > rA) { r = rB; q = lane - rA - 1; ok = rB != 0xff && q <= rB; }
+        if (!ok) { r = rA; q = 0; }
+        i = 32 * c + r; j = 32 * c + q;
+        return ok;
+    };
+#pragma unroll 1
+    for (int fi = 0; fi < nf; fi += 2) {
+        int i1, j1, i2, j2;
+        const bool ok1 = where(fi, i1, j1);
+        const bool ok2 = (fi + 1 < nf) ? where(fi + 1, i2, j2) : (where(fi, i2, j2), false);
+        const RoleI A1 = load_role_i<false, true>(s, i1);
+        const RoleJ B1 = load_role_j<false>(s, j1);
+        const RoleI A2 = load_role_i<false, true>(s, i2);
+        const RoleJ B2 = load_role_j<false>(s, j2);
+        double2 k1 = pair_kernel<false, true, true>(A1, B1, i1 - j1, pc, s);
+        double2 k2 = pair_kernel<false, true, true>(A2, B2, i2 - j2, pc, s);
+        if (i1 == j1) { k1.x *= 0.5; k1.y *= 0.5; }
+        if (i2 == j2) { k2.x *= 0.5; k2.y *= 0.5; }
+        if (ok1) f.KR[tri(i1) + j1] = k1;
+        if (ok2) f.KR[tri(i2) + j2] = k2;
+    }
+    __syncwarp();
+    const int j = 32 * c + lane;
+    const int iSj = (j < N) ? ((f.BINI[j].x >> 9) & 0x1ff) : 0;
+#pragma unroll 1
+    for (int kk = 0; kk < run.n; ++kk) {
+        uint32_t v[32];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int i = 32 * c + 8 * kk + r;
+            double2 k2 = make_double2(0.0, 0.0);
+            if (i < N && j <= i) k2 = f.KR[tri(i) + j];
+            if (i < iSj) k2.y = 0.0;
+            v[4 * r] = dlo(k2.x); v[4 * r + 1] = dhi(k2.x); v[4 * r + 2] = dlo(k2.y); v[4 * r + 3] = dhi(k2.y);
+        }
+        tmem_st32(tq + (uint32_t)(run.tcol + 32 * kk), v);
+    }
+}
+
+// ------------------------------------------------------------------------------------------ eval pieces
+// column pass of one run: lane <-> impactor column j = 32 c + lane, rows of chunks [k0, k0 + n) from tensor
+// memory; G_j += Kc_ij n_i, H_j += Kf_ij n_i (Kf already 0 where the pair does not count).
+__device__ __forceinline__ void v3_col_run(const VSm &f, const V3ColRun &run, uint32_t tq, int lane)
+{
+    uint32_t ta = tq + (uint32_t)run.tcol;
+    const double *nn = f.NN + 32 * run.c + 8 * run.k0;
+    double gc = 0.0, h = 0.0, gc2 = 0.0, h2 = 0.0;
+    // half a chunk (4 rows) per tcgen05.ld.x16; the next half is in flight while this one is summed
+    auto half = [&](const uint32_t (&v)[16], const double *n4) {
+        const double2 n01 = *reinterpret_cast<const double2 *>(n4);
+        const double2 n23 = *reinterpret_cast<const double2 *>(n4 + 2);
+        gc = fma(u2d(v[0], v[1]), n01.x, gc);      h = fma(u2d(v[2], v[3]), n01.x, h);
+        gc2 = fma(u2d(v[4], v[5]), n01.y, gc2);    h2 = fma(u2d(v[6], v[7]), n01.y, h2);
+        gc = fma(u2d(v[8], v[9]), n23.x, gc);      h = fma(u2d(v[10], v[11]), n23.x, h);
+        gc2 = fma(u2d(v[12], v[13]), n23.y, gc2);  h2 = fma(u2d(v[14], v[15]), n23.y, h2);
+    };
+    uint32_t va[16], vb[16];
+    tmem_ld16(ta, va);
+#pragma unroll 1
+    for (int kk = 0; kk < run.n; ++kk) {
+        tmem_wait_ld();
+        tmem_ld16(ta + 16, vb);
+        half(va, nn);
+        tmem_wait_ld();
+        if (kk + 1 < run.n) tmem_ld16(ta + 32, va);
+        half(vb, nn + 4);
+        ta += 32; nn += 8;
+    }
+    f.COLP[32 * run.slot + lane] = make_double2(gc + gc2, h + h2);
+}
+
+// row pass of one run: lane <-> target row i = 32 b + lane, impactor columns [ja, jb) clipped to the bulk
+// prefix j < n_bulk[i]:  A1, A2 += Kc_ij (y_j, y_j m_j);  F1, F2 += Kf_ij (y_j, y_j m_j)
+__device__ __forceinline__ void v3_row_run(const V3Tables &vt, const VSm &f, const V3RowRun &run, int lane)
+{
+    const int N = vt.N;
+    const int i = 32 * run.b + lane, iv = min(i, N - 1);
+    const int nbi = (i < N) ? (f.BINI[iv].x & 0x1ff) : 0;
+    const double2 *kr = f.KR + tri(iv);
+    const double2 *yy = f.YY;
+    double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0, b1 = 0.0, b2 = 0.0, g1 = 0.0, g2 = 0.0;
+    int j = run.ja;
+    const int jr = min((int)run.jb, vt.cmin[run.b]);
+    // the rectangle: every row of the block has these columns
+#pragma unroll 4
+    for (; j + 2 <= jr; j += 2) {
+        const double2 k2 = kr[j], k3 = kr[j + 1];
+        const double2 y2 = yy[j], y3 = yy[j + 1];
+        a1 = fma(k2.x, y2.x, a1); a2 = fma(k2.x, y2.y, a2);
+        f1 = fma(k2.y, y2.x, f1); f2 = fma(k2.y, y2.y, f2);
+        b1 = fma(k3.x, y3.x, b1); b2 = fma(k3.x, y3.y, b2);
+        g1 = fma(k3.y, y3.x, g1); g2 = fma(k3.y, y3.y, g2);
+    }
+    // the ragged rest (and an odd last rectangle column): row i takes j < n_bulk[i]; the loads are
+    // unconditional -- past the end of a row they hit the next rows of the packed array
+#pragma unroll 2
+    for (; j < run.jb; ++j) {
+        const double2 k2 = kr[j];
+        double2 y2 = yy[j];
+        if (j >= nbi) { y2.x = 0.0; y2.y = 0.0; }
+        a1 = fma(k2.x, y2.x, a1); a2 = fma(k2.x, y2.y, a2);
+        f1 = fma(k2.y, y2.x, f1); f2 = fma(k2.y, y2.y, f2);
+    }
+    double2 *pp = f.ROWP + 2 * (32 * run.slot + lane);
+    pp[0] = make_double2(a1 + b1, a2 + b2);
+    pp[1] = make_double2(f1 + g1, f2 + g2);
+}
+
+// band stencil of target block g, taps [T0, T1): lane <-> target t = 32 g + lane (coag_v3.h)
+__device__ __forceinline__ void v3_band_task(const V3Tables &vt, const VSm &f, int g, int T0, int T1, int slot,
+                                             int lane)
+{
+    const int Np = 32 * vt.nb, P = vt.P;
+    const int t = 32 * g + lane;
+    double dens = 0.0, dens2 = 0.0, S = 0.0;
+#pragma unroll 1
+    for (int q = T0; q < T1; ++q) {
+        const int d = vt.taps[q].d, o = vt.taps[q].o;
+        const double c0 = vt.taps[q].c0, c1 = vt.taps[q].c1, s1 = vt.taps[q].s1;
+        const int i = t - o, j = max(i - d, -kV3Pad);
+        const int idx = min(max(tri(i) + j, 0), P - 1);          // out of range: w == 0 (zero padding)
+        const double2 k2 = f.KR[idx];
+        const double w = f.YY[i].x * f.NN[j];
+        const double kk = fma(c0, k2.x, c1 * k2.y);
+        if (q & 1) dens2 = fma(w, kk, dens2); else dens = fma(w, kk, dens);
+        if (s1 != 0.0) S = fma(w * s1, k2.y, S);
+    }
+    dens += dens2;
+    if (slot == 0) {
+        // exception entries of the targets of this block (grid ends): lanes <-> entries, fixed xor tree
+        for (int x = 0; x < vt.nExcT; ++x) {
+            const V3ExcTarget et = vt.excT[x];
+            if ((et.t >> 5) != g) continue;
+            double tot = 0.0;
+            for (int e0 = et.e0; e0 < et.e1; e0 += 32) {
+                double v = 0.0;
+                if (e0 + lane < et.e1) {
+                    const V3Exc ex = vt.exc[e0 + lane];
+                    const double2 k2 = f.KR[tri(ex.i) + ex.j];
+                    v = (ex.coef * f.NN[ex.i]) * (f.NN[ex.j] * (ex.plane ? k2.y : k2.x));
+                }
+#pragma unroll
+                for (int m = 16; m > 0; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
+                tot += v;
+            }
+            if (lane == (et.t & 31)) { if (et.kind) S += tot; else dens += tot; }
+        }
+    }
+    double *bd = f.BAND + (size_t)slot * 2 * Np;
+    bd[t] = dens;
+    bd[Np + t] = S;
+}
+
+// ------------------------------------------------------------------------------------------ eval
+// One rate evaluation: thread k < N passes y_k and gets drho_k/dt.  mk, rmk: m_k, 1/m_k of the thread's bin.
+template <int NT>
+__device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &vt, const VSm &f, double y,
+                                          double mk, double rmk, int tid, uint32_t tbase, int ppart,
+                                          const CellGas &nx, double mu, double sigma_mol, ProlState &ps,
+                                          RoleVals &rv, int dbg = 0)
+{
+    const int N = vt.N, nb = vt.nb, Np = 32 * nb;
+    const int lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
+    const int k = tid;
+    const bool live = k < N;
+    const uint32_t tq = tq_addr(tbase, quarter, 0);
+
+    // ---- phase 0
+    double nk = 0.0;
+    if (live) {
+        nk = y * rmk;
+        f.NN[k] = nk;
+        f.YY[k] = make_double2(y, y * mk);
+    }
+    __syncthreads();
+
+    // a third of the NEXT cell's prologue per evaluation (ppart 1, 2, 3; 4: all of it), by the warps
+    // that own bins; the static schedule gives them less of the run work
+    if (ppart && warp < nb) {
+        if (ppart == 1 || ppart == 4) ps = prologue_begin(tb, nx, mu, sigma_mol, k);
+        prologue_newton(ps, ppart == 4 ? 6 : 2);
+        if (ppart >= 3) rv = prologue_finish(tb, nx, mu, ps, rmk, k);
+    }
+
+    // ---- phase A: the warp's own runs
+    if (!(dbg & 1) && vt.bandBlk[warp] >= 0) v3_band_task(vt, f, vt.bandBlk[warp], vt.bandT0[warp], vt.bandT1[warp], vt.bandSlot[warp], lane);
+#pragma unroll 1
+    for (int r = 0; r < kV3ColRuns; ++r) {
+        const V3ColRun run = vt.col[warp][r];
+        if (run.n == 0 || (dbg & 2)) break;
+        v3_col_run(f, run, tq, lane);
+    }
+#pragma unroll 1
+    for (int r = 0; r < kV3RowRuns; ++r) {
+        const V3RowRun run = vt.row[warp][r];
+        if (run.jb == run.ja || (dbg & 4)) break;
+        v3_row_run(vt, f, run, lane);
+    }
+    // per-bin constants of the combine step: in flight across the barrier
+    uint32_t cb[16];
+    uint32_t fb[2];
+    if (warp < nb) tmem_ld16(tq + (uint32_t)vt.bincCol[warp], cb);
+    else if (warp < 2 * nb) tmem_ld2(tq + (uint32_t)vt.bincCol[warp], fb);
+    __syncthreads();
+    if (warp >= 2 * nb || (dbg & 8)) return 0.0;
+
+    // ---- phase B (combine), two groups of warps side by side:
+    //   R (warp w < nb, bin 32 w + lane)     row partials -> deposits into bins k-1, k, k+1
+    //   C (warp nb + w, bin 32 w + lane)     column partials -> loss frequency G_k, fragment source of l-bin k,
+    //                                        suffix scan of S_l / B_l (Eq. 67 via l-bins)
+    double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, cFA = 0.0;
+    double *wtot = f.RED, *eUp = f.RED + 16, *eDn = f.RED + 32;
+    if (warp < nb) {
+        double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0;
+        const double2 *pp = f.ROWP + 2 * (32 * vt.rpBase[warp] + lane);
+        const int np = vt.rpCnt[warp];
+#pragma unroll 4
+        for (int p = 0; p < np; ++p) {
+            const double2 u = pp[64 * p], v = pp[64 * p + 1];
+            a1 += u.x; a2 += u.y; f1 += v.x; f2 += v.y;
+        }
+        tmem_wait_ld();
+        const double cA1 = u2d(cb[2 * VB_A1], cb[2 * VB_A1 + 1]), cA2 = u2d(cb[2 * VB_A2], cb[2 * VB_A2 + 1]);
+        const double cB1 = u2d(cb[2 * VB_B1], cb[2 * VB_B1 + 1]), cF1 = u2d(cb[2 * VB_F1], cb[2 * VB_F1 + 1]);
+        const double cF2 = u2d(cb[2 * VB_F2], cb[2 * VB_F2 + 1]), cG1 = u2d(cb[2 * VB_G1], cb[2 * VB_G1 + 1]);
+        cFA = u2d(cb[2 * VB_FA], cb[2 * VB_FA + 1]);
+        if (live) {
+            dm1 = nk * (cG1 * f1 - cF2 * f2);
+            d0 = nk * ((cA1 * a1 + cA2 * a2) + (cF1 * f1 + cF2 * f2));
+            dp1 = nk * (cB1 * a1 - cA2 * a2);
+        }
+        if (lane == 0) eDn[warp] = dm1;
+        if (lane == 31) eUp[warp] = dp1;
+    } else {
+        const int g = warp - nb, kc = 32 * g + lane;
+        auto colsum = [&](int j, double &gj, double &hj) {
+            const int c = j >> 5, np = vt.cpCnt[c];
+            const double2 *pc2 = f.COLP + 32 * vt.cpBase[c] + (j & 31);
+            gj = 0.0; hj = 0.0;
+#pragma unroll 4
+            for (int r = 0; r < np; ++r) {
+                const double2 u = pc2[32 * r];
+                gj += u.x; hj += u.y;
+            }
+        };
+        double sl = 0.0;
+        if (kc < N) {
+            const int2 bi = f.BINI[kc];
+            double gc, h;
+            colsum(kc, gc, h);
+            f.GK[kc] = gc + h;                             // G_k
+            sl = f.BAND[Np + kc] + f.BAND[3 * Np + kc];
+            for (int j = bi.y & 0xffff; j < (bi.y >> 16); ++j) {
+                double gj, hj = h;
+                if (j != kc) colsum(j, gj, hj);
+                sl = fma(tb.sS * f.YY[j].x, hj, sl);
+            }
+        }
+        tmem_wait_ld();
+        const double sv = (kc < N) ? sl * u2d(fb[0], fb[1]) : 0.0;
+        double suf = sv;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double v = __shfl_down_sync(0xffffffffu, suf, o);
+            if (lane + o < 32) suf += v;
+        }
+        if (lane == 0) wtot[g] = suf;
+        if (kc < N) f.SUF[kc] = suf;
+    }
+    const double up = __shfl_up_sync(0xffffffffu, dp1, 1);
+    const double dn = __shfl_down_sync(0xffffffffu, dm1, 1);
+    named_barrier(1, 64 * nb);
+    if (warp >= nb) return 0.0;
+
+    double d = 0.0;
+    if (live) {
+        double suf = f.SUF[k];
+        for (int w = warp + 1; w < nb; ++w) suf += wtot[w];
+        const double prev = (lane > 0) ? up : (warp > 0 ? eUp[warp - 1] : 0.0);
+        const double next = (lane < 31) ? dn : (warp + 1 < nb ? eDn[warp + 1] : 0.0);
+        d = d0;
+        if (k > 0) d += prev;
+        if (k < N - 1) d += next;
+        d += f.BAND[k] + f.BAND[2 * Np + k];
+        d = fma(-y, f.GK[k], d);
+        d = fma(cFA, suf, d);
+    }
+    return d;
+}
+
+template <int NT, int MODE>
+__global__ void __launch_bounds__(NT, 1)
+coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const StepArgs sa_in)
+{
+    StepArgs sa = sa_in;
+    if (MODE == MODE_STEP && !apply_ctrl(sa)) return;
+    extern __shared__ __align__(16) char smem_v3[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
+    const int N = vt.N, nb = vt.nb, Np = 32 * nb;
+    const VSm f = v3_carve(smem_v3, vt);
+    const Smem &s = f.s;
+    PairConst pc;
+    pc.c15vf2 = 1.5 * gs.v_frag * gs.v_frag;
+    pc.Vg2 = 0.0;
+    const int k = tid;
+    const bool live = k < N;
+
+    // ---- per-CTA constants
+    for (int q = tid; q < 64; q += NT) s.EXPT[q] = tb.exptab[q];
+    for (int q = tid; q < N; q += NT) s.DTAB[q] = tb.dtab[q];
+    for (int q = tid; q < Np; q += NT) f.BINI[q] = q < N ? tb.bini[q] : make_int2(0, 0);
+    for (int q = tid; q < Np + 2 * kV3Pad; q += NT) f.YY[q - kV3Pad] = make_double2(0.0, 0.0);
+    for (int q = tid; q < Np + 2 * kV3Pad + 8; q += NT) f.NN[q - kV3Pad] = 0.0;
+    for (int q = tid; q < 4 * Np; q += NT) f.BAND[q] = 0.0;
+    const double mk = live ? tb.binc[BC_M * tb.Np + k] : 0.0, rmk = live ? tb.binc[BC_RM * tb.Np + k] : 0.0;
+
+    uint32_t *slot = reinterpret_cast<uint32_t *>(f.RED);
+    if (tid < 32) tmem_alloc_all(slot);
+    tmem_fence_before();
+    __syncthreads();
+    tmem_fence_after();
+    const uint32_t tbase = *slot;
+    const uint32_t tq = tq_addr(tbase, quarter, 0);
+    {   // zero the whole quarter once (rows past the grid of the last chunk of a block are never written)
+        uint32_t z[32];
+#pragma unroll
+        for (int u = 0; u < 32; ++u) z[u] = 0u;
+#pragma unroll 1
+        for (int q = 0; q < 4; ++q) tmem_st32(tq + (uint32_t)(128 * (warp >> 2) + 32 * q), z);
+        tmem_wait_st();
+    }
+    tmem_fence_before();
+    __syncthreads();
+    tmem_fence_after();
+    // per-bin constants of the combine step
+    if (warp < nb) {
+        uint32_t v[16];
+#pragma unroll
+        for (int u = 0; u < 16; ++u) v[u] = 0u;
+        if (live) {
+            const int src[7] = {BC_A1, BC_A2, BC_B1, BC_F1, BC_F2, BC_G1, BC_FA};
+#pragma unroll
+            for (int u = 0; u < 7; ++u) {
+                const double c = tb.binc[src[u] * tb.Np + k];
+                v[2 * u] = dlo(c); v[2 * u + 1] = dhi(c);
+            }
+        }
+        const uint32_t t0 = tq + (uint32_t)vt.bincCol[warp];
+        const uint32_t v0[8] = {v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7]};
+        const uint32_t v1[8] = {v[8], v[9], v[10], v[11], v[12], v[13], v[14], v[15]};
+        tmem_st8(t0, v0);
+        tmem_st8(t0 + 8, v1);
+    } else if (warp < 2 * nb) {
+        const int kc = tid - 32 * nb;
+        const double c = kc < N ? tb.binc[BC_FIB * tb.Np + kc] : 0.0;
+        tmem_st2(tq + (uint32_t)vt.bincCol[warp], dlo(c), dhi(c));
+    }
+    tmem_wait_st();
+    tmem_fence_before();
+    __syncthreads();
+    tmem_fence_after();
+
+    // frozen inputs of a cell, fetched one cell ahead: the per-cell scalars at the
+    // start of the previous cell (its evaluations run the next prologue piece by piece), the per-bin
+    // velocities two evaluations before its end
+    CellGas nx = {1.0, 1.0, 1.0, 1.0};
+    double nvR = 0.0, nvZ = 0.0;
+    auto stage_gas = [&](int cell) {        // cp.async of the per-cell scalars into RED[80 .. 83]
+        if (cell >= sa.C || tid >= 4) return;
+        const double *src = tid == 0 ? gs.T : (tid == 1 ? gs.rho_g : (tid == 2 ? gs.Omega : gs.alpha));
+        if (src) cp_async8(s.RED + 80 + tid, src + cell);
+    };
+    auto take_gas = [&]() {
+        nx.T = s.RED[80]; nx.rho_g = s.RED[81]; nx.Om = s.RED[82];
+        nx.alpha = gs.alpha ? s.RED[83] : gs.alpha_const;
+    };
+    auto fetch_vel = [&](int cell) {
+        if (cell >= sa.C || !live) return;
+        const size_t g = (size_t)cell * N + k;
+        nvR = __ldg(gs.vR + g); nvZ = __ldg(gs.vZ + g);
+    };
+    stage_gas(blockIdx.x);
+    cp_async_wait_all();
+    __syncthreads();
+    take_gas();
+    fetch_vel(blockIdx.x);
+    RoleVals rv;
+    rv.Vg2 = 0.0;
+    ProlState ps = {2.0, 0.0, 0.0, 0.0};
+    bool rv_valid = false;
+
+    int err_cell = -1;          // cell whose warp error maxima wait in RED[64 ..) for the next barrier
+    auto flush_err = [&]() {
+        if (MODE == MODE_STEP && tid == 0 && err_cell >= 0) {
+            unsigned long long m = 0ull;
+            for (int w = 0; w < nb; ++w) {
+                const unsigned long long v = reinterpret_cast<const unsigned long long *>(s.RED)[64 + w];
+                m = v > m ? v : m;
+            }
+            sa.err[err_cell] = __longlong_as_double((long long)m);
+        }
+    };
+#ifdef V3_STOP
+    if (V3_STOP == 1) { __syncthreads(); if (tid < 32) tmem_dealloc_all(tbase); return; }
+#endif
+    for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
+        const size_t row = (size_t)cell * N;
+        if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, rmk, k);
+        prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
+        if (tid == 0) s.RED[95] = rv.Vg2;
+        __syncthreads();
+        pc.Vg2 = s.RED[95];
+        flush_err();
+#ifdef V3_STOP
+        if (V3_STOP == 2) { __syncthreads(); if (tid < 32) tmem_dealloc_all(tbase); return; }
+#endif
+        // state and FSAL derivative of the cell (thread <-> bin) and the next cell's gas scalars: asynchronous
+        // copies into (y, y m) -- free during the build -- and RED, landed by the post-build barrier
+        if (live) {
+            cp_async8(&f.YY[k].x, sa.rho + row + k);
+            if (MODE == MODE_STEP && sa.have_k1) cp_async8(&f.YY[k].y, sa.k_fsal + row + k);
+        }
+        stage_gas(cell + gridDim.x);
+#pragma unroll 1
+        for (int r = 0; r < kV3ColRuns; ++r) {
+            const V3ColRun run = vt.col[warp][r];
+            if (run.n == 0) break;
+            if (run.diag) v3_build_diag(vt, f, pc, run, tq, lane);
+            else v3_build_rows(vt, f, pc, run, tq, lane);
+        }
+        tmem_wait_st();
+        cp_async_wait_all();
+        double y0 = 0.0, k1 = 0.0;
+        if (live) {                                   // the thread's own copies are complete
+            y0 = f.YY[k].x;
+            if (MODE == MODE_STEP && sa.have_k1) k1 = f.YY[k].y;
+        }
+        if (MODE == MODE_STEP && warp < nb) {
+            double ws = y0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
+            if (lane == 0) s.RED[48 + warp] = ws;
+        }
+        tmem_fence_before();
+        __syncthreads();
+        tmem_fence_after();
+        take_gas();
+#ifdef V3_STOP
+        if (V3_STOP == 3) { __syncthreads(); if (tid < 32) tmem_dealloc_all(tbase); return; }
+#endif
+
+        const bool more = cell + (int)gridDim.x < sa.C;
+        if (MODE == MODE_OTF) {
+            fetch_vel(cell + gridDim.x);
+            const double d = v3_eval<NT>(tb, vt, f, y0, mk, rmk, tid, tbase, more ? 4 : 0, nx, gs.mu,
+                                         gs.sigma_mol, ps, rv, sa.Psm);
+            rv_valid = more;
+            if (live) sa.out[row + k] = d;
+            __syncthreads();
+            continue;
+        }
+
+        // ---------------- Bogacki-Shampine 3(2)
+        const double h = sa.dt;
+        double k2 = 0.0, k3 = 0.0, k4 = 0.0, yn = y0;
+#pragma unroll 1
+        for (int st = sa.have_k1 ? 1 : 0; st < 4; ++st) {
+            double ys = y0;
+            if (st == 1) ys = y0 + 0.5 * h * k1;
+            if (st == 2) ys = y0 + 0.75 * h * k2;
+            if (st == 2) fetch_vel(cell + gridDim.x);
+            if (st == 3) {
+                yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
+                ys = yn;
+            }
+            const double d = v3_eval<NT>(tb, vt, f, ys, mk, rmk, tid, tbase, more ? st : 0, nx, gs.mu,
+                                         gs.sigma_mol, ps, rv);
+            if (st == 3) rv_valid = more;
+            if (st == 0) k1 = d;
+            if (st == 1) k2 = d;
+            if (st == 2) k3 = d;
+            if (st == 3) k4 = d;
+        }
+        // error norm (R10) and write-back.  sum_k y0_k: warp sums taken before the post-build
+        // barrier; max_k: warp maxima here, combined by thread 0 after the next block barrier (the scaled
+        // errors are >= 0 or NaN, so the unsigned order of their bit patterns is the NaN-propagating max)
+        if (warp < nb) {
+            double ysum = 0.0;
+            for (int w = 0; w < nb; ++w) ysum += s.RED[48 + w];
+            const double atol = sa.atol_factor * ysum;
+            unsigned long long eb = 0ull;
+            if (live) {
+                const double e = h * ((-5.0 / 72.0) * k1 + (1.0 / 12.0) * k2 + (1.0 / 9.0) * k3 - (1.0 / 8.0) * k4);
+                const double sc = atol + sa.rtol * fmax(fabs(y0), fabs(yn));
+                const double emax = (e == 0.0) ? 0.0 : fabs(e) / sc;
+                eb = (unsigned long long)__double_as_longlong(emax);
+                sa.rho_out[row + k] = yn;
+                sa.k_out[row + k] = k4;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const unsigned long long v = __shfl_xor_sync(0xffffffffu, eb, o);
+                eb = v > eb ? v : eb;
+            }
+            if (lane == 0) reinterpret_cast<unsigned long long *>(s.RED)[64 + warp] = eb;
+        }
+        err_cell = cell;
+    }
+    tmem_fence_before();
+    __syncthreads();
+    flush_err();
+    if (tid < 32) tmem_dealloc_all(tbase);
+}
+
+template <int MODE>
+cudaError_t launch_v3_mode(const LaunchCfg &lc, const DevTables &tb, const V3Tables &vt, const GasArgs &gs,
+                           const StepArgs &sa, cudaStream_t st)
+{
+    auto fn = coag_v3_kernel<kThreads, MODE>;
+    static bool attr_done[64] = {false};    // the attribute is per device (and per instantiation)
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !attr_done[dev]) {
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, lc.smem_optin);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) attr_done[dev] = true;
+    }
+    fn<<<lc.grid, kThreads, lc.smem_bytes, st>>>(tb, vt, gs, sa);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_v3(int mode, const LaunchCfg &lc, const DevTables &tb, const V3Tables &vt,
+                      const GasArgs &gs, const StepArgs &sa, cudaStream_t st)
+{
+    if (mode == MODE_OTF) return launch_v3_mode<MODE_OTF>(lc, tb, vt, gs, sa, st);
+    return launch_v3_mode<MODE_STEP>(lc, tb, vt, gs, sa, st);
+}
+
+}  // namespace cudisc
