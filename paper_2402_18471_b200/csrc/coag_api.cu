@@ -335,7 +335,6 @@ int upload_tables(cudisc_bins b)
     V3Host V;
     v3_build(t, d.logGrid, optin, V);
     Blob bl;
-    const size_t o_vx = bl.add(V.exc);
     const size_t o_a = bl.add(t.a), o_binc = bl.add(binc), o_bini = bl.add(bini);
     const size_t o_cnt = bl.add(cnt), o_bidx = bl.add(bidx), o_bcoef = bl.add(bcoef);
     const size_t o_bI = bl.add(buildItems), o_eI = bl.add(evalItems);
@@ -356,7 +355,6 @@ int upload_tables(cudisc_bins b)
     d.sched = (const int *)(base + o_sc);
     b->dt = d;
     b->v3 = V.t;
-    b->v3.exc = (const V3Exc *)(base + o_vx);
     b->dev_blob = blob;
     b->device = dev;
     b->on_device = true;
@@ -641,10 +639,9 @@ int cudisc_bins_fast_path(cudisc_bins b, int *on, long long *smem_bytes, int *tm
     if (tmem_cols_used) {
         int used = 0;
         if (V.t.on) {
-            for (int w = 0; w < kV3Warps; ++w) {
-                used += w < V.t.nb ? 16 : (w < 2 * V.t.nb ? 2 : 0);
-                for (int r = 0; r < kV3ColRuns; ++r) used += 32 * V.t.col[w][r].n;
-            }
+            for (int w = 0; w < kV3Warps; ++w)
+                for (int r = 0; r < kV3ColRuns; ++r)
+                    if (V.t.col[w][r]) used += 32 * v3_unpack_col(V.t.col[w][r]).n;
         }
         *tmem_cols_used = used;
     }

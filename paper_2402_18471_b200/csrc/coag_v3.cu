@@ -8,12 +8,12 @@
 //     tensor memory (tcgen05.st, lane <-> column j, 8-row chunks); a 32 x 32 diagonal block is built with
 //     its short and long rows folded into full warps, then copied to tensor memory with zeros above the
 //     diagonal;
-//   * a rate evaluation reads the row copy once (row pass) and the column copy once (column pass, one
-//     tcgen05.ld.x32 per chunk, the next chunk in flight while the current one is summed);
-//   * the near-diagonal outcomes are a stencil over y_i n_{i-d} K[i][i-d] with warp-uniform coefficients
-//     from the constant bank (+ a few exception entries at the grid ends);
-//   * every warp owns a static list of runs (kernel parameter V3Tables): no queues, no atomics, fixed
-//     summation order -> results are bit-reproducible.
+//   * a rate evaluation reads the row copy once (row pass) and the column copy once (column pass,
+//     tcgen05.ld, the next half chunk in flight while the current one is summed);
+//   * the near-diagonal outcomes are a stencil over the staged products y_i n_{i-d} K[i][i-d] with
+//     warp-uniform coefficients from the constant bank (+ a few exception entries at the grid ends);
+//   * every warp owns a static list of runs (kernel parameter V3Tables, decoded into registers once): no
+//     queues, no atomics, fixed summation order -> results are bit-reproducible.
 // One persistent CTA of 512 threads per SM; thread k < N owns bin k (state and derivatives in registers).
 #include "coag_v3.h"
 #include "coag_launch.h"
@@ -27,15 +27,6 @@ __device__ __forceinline__ uint32_t tq_addr(uint32_t tbase, int quarter, int col
 {
     return tbase + ((uint32_t)(32 * quarter) << 16) + (uint32_t)col;
 }
-__device__ __forceinline__ void tmem_st2(uint32_t taddr, uint32_t a, uint32_t b)
-{
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};\n" :: "r"(taddr), "r"(a), "r"(b) : "memory");
-}
-__device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t (&v)[2])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];\n"
-                 : "=r"(v[0]), "=r"(v[1]) : "r"(taddr) : "memory");
-}
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
 {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
@@ -46,17 +37,6 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32
                     "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
                     "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
                  : "memory");
-}
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-                 "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-                   "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-                   "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-                 : "r"(taddr) : "memory");
 }
 // 8-byte asynchronous global -> shared copy (LDGSTS): inputs of a cell are staged in shared memory
 // while the build runs, without holding registers across it
@@ -69,52 +49,56 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 __device__ __forceinline__ double u2d(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
 __device__ __forceinline__ uint32_t dlo(double x) { return (uint32_t)__double2loint(x); }
 __device__ __forceinline__ uint32_t dhi(double x) { return (uint32_t)__double2hiint(x); }
-__device__ __forceinline__ void named_barrier(int id, int nthreads)
-{
-    asm volatile("bar.sync %0, %1;\n" :: "r"(id), "r"(nthreads) : "memory");
-}
 
-// per-bin constants of the combine step in tensor memory (bin-owning warps: 8 doubles in 16 columns)
-enum { VB_A1 = 0, VB_A2, VB_B1, VB_F1, VB_F2, VB_G1, VB_FA, VB_PAD, kVBinc };
+#ifdef CUDISC_PROF
+// clock64 that cannot issue before a shared-memory load issued after the barrier has returned
+__device__ __forceinline__ long long clock_after_barrier(const void *smem_word)
+{
+    long long c;
+    asm volatile("{\n .reg .pred p;\n .reg .u32 v;\n ld.volatile.shared.u32 v, [%1];\n setp.ne.u32 p, v, 0x7fc00001;\n"
+                 " mov.u64 %0, 0;\n @p mov.u64 %0, %%clock64;\n}\n"
+                 : "=l"(c) : "r"((uint32_t)__cvta_generic_to_shared(smem_word)) : "memory");
+    return c;
+}
+#define PROF_TB(var) const long long var = clock_after_barrier(f.RED())
+#define PROF_ADDB(slot, t0) do { const long long c_ = clock_after_barrier(f.RED()); if (threadIdx.x == 0) sa_prof[(slot)] += c_ - (t0); } while (0)
+#else
+#define PROF_TB(var)
+#define PROF_ADDB(slot, t0)
+#endif
 
 // ------------------------------------------------------------------------------------------ shared memory
+// Fixed arrays at compile-time offsets (coag_v3.h kV3o*): their addresses fold into the instructions.
 struct VSm {
-    double2 *KR;        // row copy of the kernel, packed lower-triangular, diagonal halved
-    double2 *YY;        // (y, y m), index -kV3Pad .. Np + kV3Pad - 1 (zeros outside the bins)
-    double *NN;         // n = y / m, same padding
-    double *RED, *BAND, *GK, *SUF;
-    int2 *BINI;
-    double2 *COLP;      // [slot][32] (G, H) partial column sums
-    double2 *ROWP;      // [slot][32][2] (A1, A2), (F1, F2) partial row sums
+    char *base;
+    double2 *KR;        // row copy of the kernel, packed lower-triangular, diagonal halved (runtime offset)
     Smem s;             // the arrays the shared device routines address (coag_device.cuh)
+    __device__ __forceinline__ double *RED() const { return reinterpret_cast<double *>(base + kV3oRED); }
+    __device__ __forceinline__ int2 *BINI() const { return reinterpret_cast<int2 *>(base + kV3oBINI); }
+    __device__ __forceinline__ double2 *YY() const { return reinterpret_cast<double2 *>(base + kV3oYY); }
+    __device__ __forceinline__ double *NN() const { return reinterpret_cast<double *>(base + kV3oNN); }
+    __device__ __forceinline__ double *BANDV() const { return reinterpret_cast<double *>(base + kV3oBANDV); }
+    __device__ __forceinline__ double *WST() const { return reinterpret_cast<double *>(base + kV3oUNION); }
+    __device__ __forceinline__ const V3Hot *HOT() const { return reinterpret_cast<const V3Hot *>(base + kV3oHOT); }
 };
 
-__device__ __forceinline__ VSm v3_carve(char *base, const V3Tables &vt)
+__device__ __forceinline__ VSm v3_carve(char *base, const DevTables &tb, const V3Tables &vt)
 {
-    const int Np = 32 * vt.nb;
     VSm f;
+    f.base = base;
     f.KR = (double2 *)(base + vt.oK);
-    f.YY = (double2 *)(base + vt.oYY) + kV3Pad;
-    f.NN = (double *)(base + vt.oNN) + kV3Pad;
-    f.RED = (double *)(base + vt.oRED);
-    f.BAND = (double *)(base + vt.oBAND);
-    f.GK = (double *)(base + vt.oGK);
-    f.SUF = f.GK + Np;
-    f.BINI = (int2 *)(base + vt.oNBULK);
-    f.COLP = (double2 *)(base + vt.oCOLP);
-    f.ROWP = (double2 *)(base + vt.oROWP);
     Smem &s = f.s;
-    double *u = (double *)(base + vt.oUNION);
-    s.YY = f.YY; s.NN = f.NN;
-    s.DTAB = (double2 *)(base + vt.oDTAB);
-    s.EXPT = (double *)(base + vt.oEXPT);
-    s.RED = f.RED;
-    s.BANDV = s.BANDV2 = nullptr; s.WST = nullptr; s.BINC = nullptr; s.BINI = f.BINI;
+    double *u = (double *)(base + kV3oUNION);
+    s.YY = f.YY(); s.NN = f.NN();
+    s.DTAB = const_cast<double2 *>(tb.dtab);      // grid-only tables of the pair kernel: read through L1
+    s.EXPT = const_cast<double *>(tb.exptab);
+    s.RED = f.RED();
+    s.BANDV = s.BANDV2 = nullptr; s.WST = nullptr; s.BINC = nullptr; s.BINI = f.BINI();
     s.CTR = nullptr; s.SCHED = nullptr; s.ITB = s.ITE = nullptr; s.PARTR = s.PARTC = nullptr;
     s.RI = (double2 *)u;
-    s.B0 = (double2 *)(u + 10 * Np); s.B1 = (double2 *)(u + 12 * Np);
-    s.J2 = (double2 *)(u + 14 * Np); s.J3 = (double2 *)(u + 16 * Np);
-    s.V5 = u + 18 * Np;
+    s.B0 = (double2 *)(u + 10 * kV3NpMax); s.B1 = (double2 *)(u + 12 * kV3NpMax);
+    s.J2 = (double2 *)(u + 14 * kV3NpMax); s.J3 = (double2 *)(u + 16 * kV3NpMax);
+    s.V5 = u + 18 * kV3NpMax;
     return f;
 }
 
@@ -128,7 +112,7 @@ __device__ __forceinline__ void v3_build_rows(const V3Tables &vt, const VSm &f, 
     const int N = vt.N;
     const int j = 32 * run.c + lane;                 // < N: the block has rows below it
     const RoleJ B = load_role_j<false>(s, j);
-    const int iSj = (f.BINI[j].x >> 9) & 0x1ff;
+    const int iSj = (f.BINI()[j].x >> 9) & 0x1ff;
     int i = 32 * run.c + 8 * run.k0;
     const int iend = min(N, i + 8 * run.n);
     uint32_t ta = tq + (uint32_t)run.tcol;
@@ -158,9 +142,9 @@ __device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, 
                                               const V3ColRun &run, uint32_t tq, int lane)
 {
     const Smem &s = f.s;
-    const int N = vt.N, c = run.c, nf = vt.nFold[c];
+    const int N = vt.N, c = run.c, nf = f.HOT()->nFold[c];
     auto where = [&](int fi, int &i, int &j) -> bool {
-        const int rA = vt.foldA[c][fi], rB = vt.foldB[c][fi];
+        const int rA = f.HOT()->foldA[c][fi], rB = f.HOT()->foldB[c][fi];
         bool ok = true;
         int r = rA, q = lane;
         if (lane > rA) { r = rB; q = lane - rA - 1; ok = rB != 0xff && q <= rB; }
@@ -186,7 +170,7 @@ __device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, 
     }
     __syncwarp();
     const int j = 32 * c + lane;
-    const int iSj = (j < N) ? ((f.BINI[j].x >> 9) & 0x1ff) : 0;
+    const int iSj = (j < N) ? ((f.BINI()[j].x >> 9) & 0x1ff) : 0;
 #pragma unroll 1
     for (int kk = 0; kk < run.n; ++kk) {
         uint32_t v[32];
@@ -205,10 +189,10 @@ __device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, 
 // ------------------------------------------------------------------------------------------ eval pieces
 // column pass of one run: lane <-> impactor column j = 32 c + lane, rows of chunks [k0, k0 + n) from tensor
 // memory; G_j += Kc_ij n_i, H_j += Kf_ij n_i (Kf already 0 where the pair does not count).
-__device__ __forceinline__ void v3_col_run(const VSm &f, const V3ColRun &run, uint32_t tq, int lane)
+__device__ __forceinline__ void v3_col_run(const V3Tables &vt, const VSm &f, const V3ColRun &run, uint32_t tq, int lane)
 {
     uint32_t ta = tq + (uint32_t)run.tcol;
-    const double *nn = f.NN + 32 * run.c + 8 * run.k0;
+    const double *nn = f.NN() + 32 * run.c + 8 * run.k0;
     double gc = 0.0, h = 0.0, gc2 = 0.0, h2 = 0.0;
     // half a chunk (4 rows) per tcgen05.ld.x16; the next half is in flight while this one is summed
     auto half = [&](const uint32_t (&v)[16], const double *n4) {
@@ -231,21 +215,27 @@ __device__ __forceinline__ void v3_col_run(const VSm &f, const V3ColRun &run, ui
         half(vb, nn + 4);
         ta += 32; nn += 8;
     }
-    f.COLP[32 * run.slot + lane] = make_double2(gc + gc2, h + h2);
+    reinterpret_cast<double2 *>(f.base + vt.oCOLP)[32 * run.slot + lane] = make_double2(gc + gc2, h + h2);
 }
 
 // row pass of one run: lane <-> target row i = 32 b + lane, impactor columns [ja, jb) clipped to the bulk
-// prefix j < n_bulk[i]:  A1, A2 += Kc_ij (y_j, y_j m_j);  F1, F2 += Kf_ij (y_j, y_j m_j)
-__device__ __forceinline__ void v3_row_run(const V3Tables &vt, const VSm &f, const V3RowRun &run, int lane)
+// prefix j < n_bulk[i]:  A1, A2 += Kc_ij (y_j, y_j m_j);  F1, F2 += Kf_ij (y_j, y_j m_j).  The slot takes
+// the deposits per unit n_i into bins i - 1, i, i + 1 (coefficients of coag_tables.h, read through L1).
+__device__ __forceinline__ void v3_row_run(const DevTables &tb, const V3Tables &vt, const VSm &f, const V3RowRun &run,
+                                           int lane)
 {
     const int N = vt.N;
     const int i = 32 * run.b + lane, iv = min(i, N - 1);
-    const int nbi = (i < N) ? (f.BINI[iv].x & 0x1ff) : 0;
+    const int nbi = (i < N) ? (f.BINI()[iv].x & 0x1ff) : 0;
+    const double *bc = tb.binc + iv;
+    const int Nq = tb.Np;
+    const double cA1 = __ldg(bc + BC_A1 * Nq), cA2 = __ldg(bc + BC_A2 * Nq), cB1 = __ldg(bc + BC_B1 * Nq);
+    const double cF1 = __ldg(bc + BC_F1 * Nq), cF2 = __ldg(bc + BC_F2 * Nq), cG1 = __ldg(bc + BC_G1 * Nq);
     const double2 *kr = f.KR + tri(iv);
-    const double2 *yy = f.YY;
+    const double2 *yy = f.YY();
     double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0, b1 = 0.0, b2 = 0.0, g1 = 0.0, g2 = 0.0;
     int j = run.ja;
-    const int jr = min((int)run.jb, vt.cmin[run.b]);
+    const int jr = min(run.jb, f.HOT()->cmin[run.b]);
     // the rectangle: every row of the block has these columns
 #pragma unroll 4
     for (; j + 2 <= jr; j += 2) {
@@ -258,149 +248,173 @@ __device__ __forceinline__ void v3_row_run(const V3Tables &vt, const VSm &f, con
     }
     // the ragged rest (and an odd last rectangle column): row i takes j < n_bulk[i]; the loads are
     // unconditional -- past the end of a row they hit the next rows of the packed array
-#pragma unroll 2
+#pragma unroll 4
     for (; j < run.jb; ++j) {
         const double2 k2 = kr[j];
         double2 y2 = yy[j];
-        if (j >= nbi) { y2.x = 0.0; y2.y = 0.0; }
+        const bool on = j < nbi;                     // (selects, not branches: the warp stays converged)
+        y2.x = on ? y2.x : 0.0; y2.y = on ? y2.y : 0.0;
         a1 = fma(k2.x, y2.x, a1); a2 = fma(k2.x, y2.y, a2);
         f1 = fma(k2.y, y2.x, f1); f2 = fma(k2.y, y2.y, f2);
     }
-    double2 *pp = f.ROWP + 2 * (32 * run.slot + lane);
-    pp[0] = make_double2(a1 + b1, a2 + b2);
-    pp[1] = make_double2(f1 + g1, f2 + g2);
+    a1 += b1; a2 += b2; f1 += g1; f2 += g2;
+    double *pp = reinterpret_cast<double *>(f.base + vt.oROWP) + 96 * run.slot + lane;
+    pp[0] = cG1 * f1 - cF2 * f2;                                     // -> bin i - 1
+    pp[32] = (cA1 * a1 + cA2 * a2) + (cF1 * f1 + cF2 * f2);          // -> bin i
+    pp[64] = cB1 * a1 - cA2 * a2;                                    // -> bin i + 1
 }
 
-// band stencil of target block g, taps [T0, T1): lane <-> target t = 32 g + lane (coag_v3.h)
-__device__ __forceinline__ void v3_band_task(const V3Tables &vt, const VSm &f, int g, int T0, int T1, int slot,
-                                             int lane)
+// band stage of the bins 32 g + lane (coag_v3.h): W[plane][d][i] = y_i n_{i-d} Kplane[i][i-d], 0 where the
+// pair does not exist; yi: the thread's own y (0 for i >= N)
+__device__ __forceinline__ void v3_stage(const V3Tables &vt, const VSm &f, int i, double yi)
 {
-    const int Np = 32 * vt.nb, P = vt.P;
-    const int t = 32 * g + lane;
-    double dens = 0.0, dens2 = 0.0, S = 0.0;
-#pragma unroll 1
-    for (int q = T0; q < T1; ++q) {
-        const int d = vt.taps[q].d, o = vt.taps[q].o;
-        const double c0 = vt.taps[q].c0, c1 = vt.taps[q].c1, s1 = vt.taps[q].s1;
-        const int i = t - o, j = max(i - d, -kV3Pad);
-        const int idx = min(max(tri(i) + j, 0), P - 1);          // out of range: w == 0 (zero padding)
-        const double2 k2 = f.KR[idx];
-        const double w = f.YY[i].x * f.NN[j];
-        const double kk = fma(c0, k2.x, c1 * k2.y);
-        if (q & 1) dens2 = fma(w, kk, dens2); else dens = fma(w, kk, dens);
-        if (s1 != 0.0) S = fma(w * s1, k2.y, S);
-    }
-    dens += dens2;
-    if (slot == 0) {
-        // exception entries of the targets of this block (grid ends): lanes <-> entries, fixed xor tree
-        for (int x = 0; x < vt.nExcT; ++x) {
-            const V3ExcTarget et = vt.excT[x];
-            if ((et.t >> 5) != g) continue;
-            double tot = 0.0;
-            for (int e0 = et.e0; e0 < et.e1; e0 += 32) {
-                double v = 0.0;
-                if (e0 + lane < et.e1) {
-                    const V3Exc ex = vt.exc[e0 + lane];
-                    const double2 k2 = f.KR[tri(ex.i) + ex.j];
-                    v = (ex.coef * f.NN[ex.i]) * (f.NN[ex.j] * (ex.plane ? k2.y : k2.x));
-                }
-#pragma unroll
-                for (int m = 16; m > 0; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
-                tot += v;
-            }
-            if (lane == (et.t & 31)) { if (et.kind) S += tot; else dens += tot; }
+    const int N = vt.N, D = vt.bandD;
+    const int iv = min(i, N - 1);
+    const double2 *kr = f.KR + tri(iv) + iv;
+    const double *nn = f.NN() + iv;
+    double *w = f.WST() + vt.wPad + i;
+    const int plane = D * vt.wRow;
+#pragma unroll 2
+    for (int d = 0; d < D; ++d) {
+        double wc = 0.0, wf = 0.0;
+        if (d <= iv) {
+            const double2 k2 = kr[-d];
+            const double yn = yi * nn[-d];
+            wc = yn * k2.x; wf = yn * k2.y;
         }
+        w[d * vt.wRow] = wc;
+        w[plane + d * vt.wRow] = wf;
     }
-    double *bd = f.BAND + (size_t)slot * 2 * Np;
-    bd[t] = dens;
-    bd[Np + t] = S;
+}
+
+// exception entries of target block g, kind `kind` (grid ends; coag_v3.h): lanes <-> entries of one target, fixed
+// xor tree, the lane that owns the target adds the sum
+__device__ __forceinline__ double v3_exceptions(const VSm &f, const double *wst, int g, int kind, int lane, double acc)
+{
+    const V3Hot *hot = f.HOT();
+#pragma unroll 1
+    for (int x = 0; x < kV3MaxExcT; ++x) {
+        const V3ExcTarget et = hot->excT[x];
+        if (et.t < 0) break;
+        if (et.kind != kind || (et.t >> 5) != g) continue;
+        double v = 0.0;
+        if (et.e0 + lane < et.e1) v = hot->exc[et.e0 + lane].c * wst[hot->exc[et.e0 + lane].off];
+#pragma unroll
+        for (int m = 16; m > 0; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
+        if (lane == (et.t & 31)) acc += v;
+    }
+    return acc;
+}
+
+// band stencil of target t over taps [q0, q1) (multiples of 4): 4 loads in flight per batch
+__device__ __forceinline__ double v3_taps(const VSm &f, const double *wst, int t, int q0, int q1)
+{
+    const V3Hot *hot = f.HOT();
+    double da = 0.0, db = 0.0;
+#pragma unroll 1
+    for (int q = q0; q < q1; q += 4) {
+        double w4[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) w4[u] = wst[hot->taps[q + u].off + t];
+        da = fma(hot->taps[q].c, w4[0], da);
+        db = fma(hot->taps[q + 1].c, w4[1], db);
+        da = fma(hot->taps[q + 2].c, w4[2], da);
+        db = fma(hot->taps[q + 3].c, w4[3], db);
+    }
+    return da + db;
 }
 
 // ------------------------------------------------------------------------------------------ eval
-// One rate evaluation: thread k < N passes y_k and gets drho_k/dt.  mk, rmk: m_k, 1/m_k of the thread's bin.
+// One rate evaluation: thread k < N passes y_k and gets drho_k/dt.  c1, c2, c3: per-thread constants of the
+// thread's role -- bin owners (warp < nb): m_k, 1 / m_k, A_k; column-combine group (warp nb + g): -, -, 1 / B_k.
 template <int NT>
 __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &vt, const VSm &f, double y,
-                                          double mk, double rmk, int tid, uint32_t tbase, int ppart,
+                                          double c1, double c2, double c3, int tid, uint32_t tq, int ppart,
                                           const CellGas &nx, double mu, double sigma_mol, ProlState &ps,
-                                          RoleVals &rv, int dbg = 0)
+                                          RoleVals &rv, const uint32_t (&colw)[kV3ColRuns],
+                                          const uint32_t (&roww)[kV3RowRuns], int dbg)
 {
-    const int N = vt.N, nb = vt.nb, Np = 32 * nb;
-    const int lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
+    const int N = vt.N, nb = vt.nb;
+    const int lane = tid & 31, warp = tid >> 5;
     const int k = tid;
     const bool live = k < N;
-    const uint32_t tq = tq_addr(tbase, quarter, 0);
+    long long *sa_prof = reinterpret_cast<long long *>(f.RED() + 96);
+    (void)sa_prof;
+    PROF_T(tp0);
 
     // ---- phase 0
     double nk = 0.0;
     if (live) {
-        nk = y * rmk;
-        f.NN[k] = nk;
-        f.YY[k] = make_double2(y, y * mk);
+        nk = y * c2;
+        f.NN()[k] = nk;
+        f.YY()[k] = make_double2(y, y * c1);
     }
     __syncthreads();
+    PROF_ADDB(2, tp0);
+    PROF_TB(tpA);
 
-    // a third of the NEXT cell's prologue per evaluation (ppart 1, 2, 3; 4: all of it), by the warps
-    // that own bins; the static schedule gives them less of the run work
-    if (ppart && warp < nb) {
-        if (ppart == 1 || ppart == 4) ps = prologue_begin(tb, nx, mu, sigma_mol, k);
-        prologue_newton(ps, ppart == 4 ? 6 : 2);
-        if (ppart >= 3) rv = prologue_finish(tb, nx, mu, ps, rmk, k);
+    // ---- phase A: the bin-owning warps stage the band products of their bins and run a third of the NEXT
+    //      cell's prologue (ppart 1, 2, 3; 4: all of it); then every warp its own runs
+    if (warp < nb) {
+        if (!(dbg & 1)) v3_stage(vt, f, k, live ? y : 0.0);
+        if (ppart) {
+            if (ppart == 1 || ppart == 4) ps = prologue_begin(tb, nx, mu, sigma_mol, k);
+            prologue_newton(ps, ppart == 4 ? 6 : 2);
+            if (ppart >= 3) rv = prologue_finish(tb, nx, mu, ps, c2, k);
+        }
     }
-
-    // ---- phase A: the warp's own runs
-    if (!(dbg & 1) && vt.bandBlk[warp] >= 0) v3_band_task(vt, f, vt.bandBlk[warp], vt.bandT0[warp], vt.bandT1[warp], vt.bandSlot[warp], lane);
+    // (one copy of each run body: the instruction cache matters more than the select chain.  Column runs
+    //  first on every warp: starting odd warps on their row runs instead was measured slower)
 #pragma unroll 1
     for (int r = 0; r < kV3ColRuns; ++r) {
-        const V3ColRun run = vt.col[warp][r];
-        if (run.n == 0 || (dbg & 2)) break;
-        v3_col_run(f, run, tq, lane);
+        const uint32_t w = r == 0 ? colw[0] : (r == 1 ? colw[1] : (r == 2 ? colw[2] : colw[3]));
+        if (!w || (dbg & 2)) break;
+        v3_col_run(vt, f, v3_unpack_col(w), tq, lane);
     }
 #pragma unroll 1
     for (int r = 0; r < kV3RowRuns; ++r) {
-        const V3RowRun run = vt.row[warp][r];
-        if (run.jb == run.ja || (dbg & 4)) break;
-        v3_row_run(vt, f, run, lane);
+        const uint32_t w = r == 0 ? roww[0] : (r == 1 ? roww[1] : roww[2]);
+        if (!w || (dbg & 4)) break;
+        v3_row_run(tb, vt, f, v3_unpack_row(w), lane);
     }
-    // per-bin constants of the combine step: in flight across the barrier
-    uint32_t cb[16];
-    uint32_t fb[2];
-    if (warp < nb) tmem_ld16(tq + (uint32_t)vt.bincCol[warp], cb);
-    else if (warp < 2 * nb) tmem_ld2(tq + (uint32_t)vt.bincCol[warp], fb);
+    PROF_ADD(3, tpA);
+#ifdef CUDISC_PROF
+    if (lane == 0) sa_prof[16 + warp] += clock64() - tpA;     // RED[112 ..]: per-warp busy time of phase A
+#endif
     __syncthreads();
-    if (warp >= 2 * nb || (dbg & 8)) return 0.0;
+    PROF_ADDB(4, tpA);
+    PROF_TB(tpB);
 
-    // ---- phase B (combine), two groups of warps side by side:
-    //   R (warp w < nb, bin 32 w + lane)     row partials -> deposits into bins k-1, k, k+1
-    //   C (warp nb + w, bin 32 w + lane)     column partials -> loss frequency G_k, fragment source of l-bin k,
-    //                                        suffix scan of S_l / B_l (Eq. 67 via l-bins)
-    double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, cFA = 0.0;
-    double *wtot = f.RED, *eUp = f.RED + 16, *eDn = f.RED + 32;
-    if (warp < nb) {
-        double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0;
-        const double2 *pp = f.ROWP + 2 * (32 * vt.rpBase[warp] + lane);
-        const int np = vt.rpCnt[warp];
+    // ---- phase B (combine), three groups of warps side by side:
+    //   R (warp w < nb, bin 32 w + lane)      row partials -> deposits into bins k-1, k, k+1; first half of the
+    //                                         band stencil of its bins (stays in a register)
+    //   C (warp nb + w, bin 32 w + lane)      column partials -> loss frequency G_k, fragment source of l-bin k,
+    //                                         suffix scan of S_l / B_l (Eq. 67 via l-bins)
+    //   D (warp 2 nb + w, bin 32 w + lane)    second half of the band stencil, exception entries -> BANDV
+    // G_k and the scanned value travel through NN[k] and YY[k].y, dead by now.
+    double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, up = 0.0, dn = 0.0, bandR = 0.0;
+    double *wtot = f.RED(), *eUp = f.RED() + 16, *eDn = f.RED() + 32;
+    const double *wst = f.WST();
+    if (dbg & 8) {
+    } else if (warp < nb) {
+        const double *pp = reinterpret_cast<const double *>(f.base + vt.oROWP) + 96 * f.HOT()->rpBase[warp] + lane;
+        const int np = f.HOT()->rpCnt[warp];
 #pragma unroll 4
         for (int p = 0; p < np; ++p) {
-            const double2 u = pp[64 * p], v = pp[64 * p + 1];
-            a1 += u.x; a2 += u.y; f1 += v.x; f2 += v.y;
+            dm1 += pp[96 * p]; d0 += pp[96 * p + 32]; dp1 += pp[96 * p + 64];
         }
-        tmem_wait_ld();
-        const double cA1 = u2d(cb[2 * VB_A1], cb[2 * VB_A1 + 1]), cA2 = u2d(cb[2 * VB_A2], cb[2 * VB_A2 + 1]);
-        const double cB1 = u2d(cb[2 * VB_B1], cb[2 * VB_B1 + 1]), cF1 = u2d(cb[2 * VB_F1], cb[2 * VB_F1 + 1]);
-        const double cF2 = u2d(cb[2 * VB_F2], cb[2 * VB_F2 + 1]), cG1 = u2d(cb[2 * VB_G1], cb[2 * VB_G1 + 1]);
-        cFA = u2d(cb[2 * VB_FA], cb[2 * VB_FA + 1]);
-        if (live) {
-            dm1 = nk * (cG1 * f1 - cF2 * f2);
-            d0 = nk * ((cA1 * a1 + cA2 * a2) + (cF1 * f1 + cF2 * f2));
-            dp1 = nk * (cB1 * a1 - cA2 * a2);
-        }
+        dm1 *= nk; d0 *= nk; dp1 *= nk;
         if (lane == 0) eDn[warp] = dm1;
         if (lane == 31) eUp[warp] = dp1;
-    } else {
+        up = __shfl_up_sync(0xffffffffu, dp1, 1);
+        dn = __shfl_down_sync(0xffffffffu, dm1, 1);
+        bandR = v3_taps(f, wst, k, 0, vt.nTaps >> 1);
+    } else if (warp < 2 * nb) {
         const int g = warp - nb, kc = 32 * g + lane;
+        const double2 *colp = reinterpret_cast<const double2 *>(f.base + vt.oCOLP);
         auto colsum = [&](int j, double &gj, double &hj) {
-            const int c = j >> 5, np = vt.cpCnt[c];
-            const double2 *pc2 = f.COLP + 32 * vt.cpBase[c] + (j & 31);
+            const int c = j >> 5, np = f.HOT()->cpCnt[c];
+            const double2 *pc2 = colp + 32 * f.HOT()->cpBase[c] + (j & 31);
             gj = 0.0; hj = 0.0;
 #pragma unroll 4
             for (int r = 0; r < np; ++r) {
@@ -409,20 +423,23 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
             }
         };
         double sl = 0.0;
+        {   // S stencil of l-bin kc (stage entries past the bins are 0) and its exceptions
+#pragma unroll 1
+            for (int q = 0; q < vt.nSTaps; ++q) sl = fma(f.HOT()->staps[q].c, wst[f.HOT()->staps[q].off + kc], sl);
+        }
+        sl = v3_exceptions(f, wst, g, 1, lane, sl);
         if (kc < N) {
-            const int2 bi = f.BINI[kc];
+            const int2 bi = f.BINI()[kc];
             double gc, h;
             colsum(kc, gc, h);
-            f.GK[kc] = gc + h;                             // G_k
-            sl = f.BAND[Np + kc] + f.BAND[3 * Np + kc];
+            f.NN()[kc] = gc + h;                           // G_k
             for (int j = bi.y & 0xffff; j < (bi.y >> 16); ++j) {
                 double gj, hj = h;
                 if (j != kc) colsum(j, gj, hj);
-                sl = fma(tb.sS * f.YY[j].x, hj, sl);
+                sl = fma(tb.sS * f.YY()[j].x, hj, sl);
             }
         }
-        tmem_wait_ld();
-        const double sv = (kc < N) ? sl * u2d(fb[0], fb[1]) : 0.0;
+        const double sv = (kc < N) ? sl * c3 : 0.0;
         double suf = sv;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -430,26 +447,41 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
             if (lane + o < 32) suf += v;
         }
         if (lane == 0) wtot[g] = suf;
-        if (kc < N) f.SUF[kc] = suf;
+        if (kc < N) f.YY()[kc].y = suf;
+#ifdef CUDISC_PROF
+        if (tid == 32 * nb) sa_prof[9] += clock64() - tpB;
+#endif
+    } else if (warp < 3 * nb) {
+#ifdef CUDISC_PROF
+        if (tid == 64 * nb) sa_prof[13] += clock64() - tpB;
+#endif
+        const int g = warp - 2 * nb, t = 32 * g + lane;
+        double da = v3_taps(f, wst, t, vt.nTaps >> 1, vt.nTaps);       // (the list is padded to a multiple of 8)
+        da = v3_exceptions(f, wst, g, 0, lane, da);
+        f.BANDV()[t] = da;
+#ifdef CUDISC_PROF
+        if (tid == 64 * nb) sa_prof[10] += clock64() - tpB;
+#endif
     }
-    const double up = __shfl_up_sync(0xffffffffu, dp1, 1);
-    const double dn = __shfl_down_sync(0xffffffffu, dm1, 1);
-    named_barrier(1, 64 * nb);
+    PROF_ADD(5, tpB);
+    __syncthreads();
+    PROF_ADDB(7, tpB);
     if (warp >= nb) return 0.0;
 
     double d = 0.0;
     if (live) {
-        double suf = f.SUF[k];
+        double suf = f.YY()[k].y;
         for (int w = warp + 1; w < nb; ++w) suf += wtot[w];
         const double prev = (lane > 0) ? up : (warp > 0 ? eUp[warp - 1] : 0.0);
         const double next = (lane < 31) ? dn : (warp + 1 < nb ? eDn[warp + 1] : 0.0);
         d = d0;
         if (k > 0) d += prev;
         if (k < N - 1) d += next;
-        d += f.BAND[k] + f.BAND[2 * Np + k];
-        d = fma(-y, f.GK[k], d);
-        d = fma(cFA, suf, d);
+        d += bandR + f.BANDV()[k];
+        d = fma(-y, f.NN()[k], d);
+        d = fma(c3, suf, d);
     }
+    PROF_ADD(6, tpB);
     return d;
 }
 
@@ -461,25 +493,37 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     if (MODE == MODE_STEP && !apply_ctrl(sa)) return;
     extern __shared__ __align__(16) char smem_v3[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
-    const int N = vt.N, nb = vt.nb, Np = 32 * nb;
-    const VSm f = v3_carve(smem_v3, vt);
+    const int N = vt.N, nb = vt.nb;
+    const VSm f = v3_carve(smem_v3, tb, vt);
     const Smem &s = f.s;
     PairConst pc;
     pc.c15vf2 = 1.5 * gs.v_frag * gs.v_frag;
     pc.Vg2 = 0.0;
     const int k = tid;
     const bool live = k < N;
+    const int dbg = sa.Psm;
 
     // ---- per-CTA constants
-    for (int q = tid; q < 64; q += NT) s.EXPT[q] = tb.exptab[q];
-    for (int q = tid; q < N; q += NT) s.DTAB[q] = tb.dtab[q];
-    for (int q = tid; q < Np; q += NT) f.BINI[q] = q < N ? tb.bini[q] : make_int2(0, 0);
-    for (int q = tid; q < Np + 2 * kV3Pad; q += NT) f.YY[q - kV3Pad] = make_double2(0.0, 0.0);
-    for (int q = tid; q < Np + 2 * kV3Pad + 8; q += NT) f.NN[q - kV3Pad] = 0.0;
-    for (int q = tid; q < 4 * Np; q += NT) f.BAND[q] = 0.0;
-    const double mk = live ? tb.binc[BC_M * tb.Np + k] : 0.0, rmk = live ? tb.binc[BC_RM * tb.Np + k] : 0.0;
+    for (int q = tid; q < kV3NpMax; q += NT) f.BINI()[q] = q < N ? tb.bini[q] : make_int2(0, 0);
+    for (int q = tid; q < kV3NpMax; q += NT) f.YY()[q] = make_double2(0.0, 0.0);
+    for (int q = tid; q < kV3NpMax + 16; q += NT) f.NN()[q] = 0.0;
+    for (int q = tid; q < kV3NpMax; q += NT) f.BANDV()[q] = 0.0;
+    for (int q = tid; q < (int)(sizeof(V3Hot) / 4); q += NT)
+        reinterpret_cast<uint32_t *>(smem_v3 + kV3oHOT)[q] = reinterpret_cast<const uint32_t *>(&vt.hot)[q];
+    // the thread's runs (kernel parameters -> registers) and the constants of its role (v3_eval)
+    uint32_t colw[kV3ColRuns], roww[kV3RowRuns];
+#pragma unroll
+    for (int r = 0; r < kV3ColRuns; ++r) colw[r] = vt.col[warp][r];
+#pragma unroll
+    for (int r = 0; r < kV3RowRuns; ++r) roww[r] = vt.row[warp][r];
+    double c1 = 0.0, c2 = 0.0, c3 = 0.0;
+    if (live) {
+        c1 = tb.binc[BC_M * tb.Np + k]; c2 = tb.binc[BC_RM * tb.Np + k]; c3 = tb.binc[BC_FA * tb.Np + k];
+    } else if (warp >= nb && warp < 2 * nb && tid - 32 * nb < N) {
+        c3 = tb.binc[BC_FIB * tb.Np + tid - 32 * nb];
+    }
 
-    uint32_t *slot = reinterpret_cast<uint32_t *>(f.RED);
+    uint32_t *slot = reinterpret_cast<uint32_t *>(f.RED());
     if (tid < 32) tmem_alloc_all(slot);
     tmem_fence_before();
     __syncthreads();
@@ -494,33 +538,6 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         for (int q = 0; q < 4; ++q) tmem_st32(tq + (uint32_t)(128 * (warp >> 2) + 32 * q), z);
         tmem_wait_st();
     }
-    tmem_fence_before();
-    __syncthreads();
-    tmem_fence_after();
-    // per-bin constants of the combine step
-    if (warp < nb) {
-        uint32_t v[16];
-#pragma unroll
-        for (int u = 0; u < 16; ++u) v[u] = 0u;
-        if (live) {
-            const int src[7] = {BC_A1, BC_A2, BC_B1, BC_F1, BC_F2, BC_G1, BC_FA};
-#pragma unroll
-            for (int u = 0; u < 7; ++u) {
-                const double c = tb.binc[src[u] * tb.Np + k];
-                v[2 * u] = dlo(c); v[2 * u + 1] = dhi(c);
-            }
-        }
-        const uint32_t t0 = tq + (uint32_t)vt.bincCol[warp];
-        const uint32_t v0[8] = {v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7]};
-        const uint32_t v1[8] = {v[8], v[9], v[10], v[11], v[12], v[13], v[14], v[15]};
-        tmem_st8(t0, v0);
-        tmem_st8(t0 + 8, v1);
-    } else if (warp < 2 * nb) {
-        const int kc = tid - 32 * nb;
-        const double c = kc < N ? tb.binc[BC_FIB * tb.Np + kc] : 0.0;
-        tmem_st2(tq + (uint32_t)vt.bincCol[warp], dlo(c), dhi(c));
-    }
-    tmem_wait_st();
     tmem_fence_before();
     __syncthreads();
     tmem_fence_after();
@@ -565,31 +582,34 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             sa.err[err_cell] = __longlong_as_double((long long)m);
         }
     };
-#ifdef V3_STOP
-    if (V3_STOP == 1) { __syncthreads(); if (tid < 32) tmem_dealloc_all(tbase); return; }
+#ifdef CUDISC_PROF
+    long long *sa_prof = reinterpret_cast<long long *>(f.RED() + 96);
+    if (tid < 32) sa_prof[tid] = 0;
+    __syncthreads();
 #endif
     for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
+        PROF_T(tc0);
         const size_t row = (size_t)cell * N;
-        if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, rmk, k);
+        if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, c2, k);
         prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
         if (tid == 0) s.RED[95] = rv.Vg2;
         __syncthreads();
         pc.Vg2 = s.RED[95];
         flush_err();
-#ifdef V3_STOP
-        if (V3_STOP == 2) { __syncthreads(); if (tid < 32) tmem_dealloc_all(tbase); return; }
-#endif
+        PROF_ADD(0, tc0);
+        PROF_T(tb0);
         // state and FSAL derivative of the cell (thread <-> bin) and the next cell's gas scalars: asynchronous
         // copies into (y, y m) -- free during the build -- and RED, landed by the post-build barrier
         if (live) {
-            cp_async8(&f.YY[k].x, sa.rho + row + k);
-            if (MODE == MODE_STEP && sa.have_k1) cp_async8(&f.YY[k].y, sa.k_fsal + row + k);
+            cp_async8(&f.YY()[k].x, sa.rho + row + k);
+            if (MODE == MODE_STEP && sa.have_k1) cp_async8(&f.YY()[k].y, sa.k_fsal + row + k);
         }
         stage_gas(cell + gridDim.x);
 #pragma unroll 1
         for (int r = 0; r < kV3ColRuns; ++r) {
-            const V3ColRun run = vt.col[warp][r];
-            if (run.n == 0) break;
+            const uint32_t w = r == 0 ? colw[0] : (r == 1 ? colw[1] : (r == 2 ? colw[2] : colw[3]));
+            if (!w) break;
+            const V3ColRun run = v3_unpack_col(w);
             if (run.diag) v3_build_diag(vt, f, pc, run, tq, lane);
             else v3_build_rows(vt, f, pc, run, tq, lane);
         }
@@ -597,8 +617,8 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         cp_async_wait_all();
         double y0 = 0.0, k1 = 0.0;
         if (live) {                                   // the thread's own copies are complete
-            y0 = f.YY[k].x;
-            if (MODE == MODE_STEP && sa.have_k1) k1 = f.YY[k].y;
+            y0 = f.YY()[k].x;
+            if (MODE == MODE_STEP && sa.have_k1) k1 = f.YY()[k].y;
         }
         if (MODE == MODE_STEP && warp < nb) {
             double ws = y0;
@@ -610,15 +630,22 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         __syncthreads();
         tmem_fence_after();
         take_gas();
-#ifdef V3_STOP
-        if (V3_STOP == 3) { __syncthreads(); if (tid < 32) tmem_dealloc_all(tbase); return; }
-#endif
+        PROF_ADDB(11, tb0);
+        // the role vectors are dead: zero the padding of the band stage (its bins are written per evaluation)
+        {
+            const int padB = vt.wRow - vt.wPad - 32 * nb, npad = vt.wPad + padB, rows = 2 * vt.bandD;
+            for (int q = tid; q < rows * npad; q += NT) {
+                const int r = q / npad, e = q - r * npad;
+                f.WST()[r * vt.wRow + (e < vt.wPad ? e : 32 * nb + e)] = 0.0;
+            }
+        }
+        PROF_ADD(1, tb0);
 
         const bool more = cell + (int)gridDim.x < sa.C;
         if (MODE == MODE_OTF) {
             fetch_vel(cell + gridDim.x);
-            const double d = v3_eval<NT>(tb, vt, f, y0, mk, rmk, tid, tbase, more ? 4 : 0, nx, gs.mu,
-                                         gs.sigma_mol, ps, rv, sa.Psm);
+            const double d = v3_eval<NT>(tb, vt, f, y0, c1, c2, c3, tid, tq, more ? 4 : 0, nx, gs.mu,
+                                         gs.sigma_mol, ps, rv, colw, roww, dbg);
             rv_valid = more;
             if (live) sa.out[row + k] = d;
             __syncthreads();
@@ -638,8 +665,8 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
                 yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
                 ys = yn;
             }
-            const double d = v3_eval<NT>(tb, vt, f, ys, mk, rmk, tid, tbase, more ? st : 0, nx, gs.mu,
-                                         gs.sigma_mol, ps, rv);
+            const double d = v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nx, gs.mu,
+                                         gs.sigma_mol, ps, rv, colw, roww, dbg);
             if (st == 3) rv_valid = more;
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;
@@ -670,10 +697,14 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             if (lane == 0) reinterpret_cast<unsigned long long *>(s.RED)[64 + warp] = eb;
         }
         err_cell = cell;
+        PROF_ADD(8, tc0);
     }
     tmem_fence_before();
     __syncthreads();
     flush_err();
+#ifdef CUDISC_PROF
+    if (tid < 32 && sa.prof) sa.prof[48 * (size_t)blockIdx.x + tid] += sa_prof[tid];
+#endif
     if (tid < 32) tmem_dealloc_all(tbase);
 }
 

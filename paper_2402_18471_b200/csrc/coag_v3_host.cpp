@@ -15,10 +15,10 @@ namespace {
 
 // cost model (cycles of one warp; measured ratios on B200, only the ratios matter)
 constexpr double kCBuildRow = 95.0, kCBuildFold = 120.0, kCBuildDiagCopy = 320.0;
-constexpr double kCColChunk = 70.0, kCColRun = 90.0;
-constexpr double kCRowRect = 24.0, kCRowRag = 32.0, kCRowRun = 110.0;
-constexpr double kCTap = 50.0, kCBandTask = 150.0, kCExcTarget = 260.0;
-constexpr double kCProlPiece = 700.0;     // a third of the next cell's prologue, on the bin-owning warps
+constexpr double kCColChunk = 450.0, kCColRun = 150.0;
+constexpr double kCRowRect = 70.0, kCRowRag = 110.0, kCRowRun = 300.0;
+constexpr double kCStage = 500.0;          // band stage of the warp's own bins
+constexpr double kCProlPiece = 1700.0;     // a third of the next cell's prologue, on the bin-owning warps
 
 struct Key {
     int kind, d, plane, o;
@@ -31,7 +31,6 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
 {
     V3Tables &t = out.t;
     memset(&t, 0, sizeof(t));
-    out.exc.clear();
     out.why.clear();
     const int N = ht.N, nb = (N + 31) / 32, P = N * (N + 1) / 2, Np = 32 * nb;
     if (!logGrid) { out.why = "not an exact log grid"; return; }
@@ -52,7 +51,7 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
         const int kind = std::get<0>(kv.first), tb = std::get<1>(kv.first), i = std::get<2>(kv.first);
         ratio[{kind, i - std::get<3>(kv.first), std::get<4>(kv.first), tb - i}].push_back(kv.second / ht.m[i]);
     }
-    if (maxd >= kV3Pad) { out.why = "band wider than the stencil padding"; return; }
+    if (maxd >= 8) { out.why = "band wider than 8 diagonals"; return; }
     std::map<Key, double> cc;                      // class constant of the regular classes
     for (auto &kv : ratio) {
         if (kv.first.kind == 1 && kv.first.plane == 0) { out.why = "S entry on the coagulation plane"; return; }
@@ -61,37 +60,45 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
         std::sort(v.begin(), v.end());
         cc[kv.first] = v[v.size() / 2];
     }
-    std::map<std::pair<int, int>, V3Tap> tapmap;   // (d, o)
-    for (auto &kv : cc) {
+    int omin = 0, omax = 0;
+    for (auto &kv : cc) { omin = std::min(omin, kv.first.o); omax = std::max(omax, kv.first.o); }
+    const int D = maxd + 1;
+    t.bandD = D;
+    t.wPad = (omax + 1) & ~1;
+    t.wRow = (t.wPad + Np + (-omin) + 1) & ~1;
+    if (2 * D * t.wRow > 32000) { out.why = "band stage too large"; return; }
+    t.nTaps = t.nSTaps = 0;
+    for (auto &kv : cc) {                          // sorted by (kind, d, plane, o): fixed summation order
         const Key &k = kv.first;
-        if (std::abs(k.o) >= kV3Pad) { out.why = "stencil offset beyond the padding"; return; }
-        V3Tap &tp = tapmap[{k.d, k.o}];
-        tp.d = k.d; tp.o = k.o;
-        if (k.kind == 0 && k.plane == 0) tp.c0 = kv.second;
-        else if (k.kind == 0) tp.c1 = kv.second;
-        else tp.s1 = kv.second;
-    }
-    if ((int)tapmap.size() > kV3MaxTaps) { out.why = "too many stencil taps"; return; }
-    // residuals: what the taps add at (kind, target, i, j, plane), against what the table says
-    for (auto &kv : tapmap) {
-        const V3Tap &tp = kv.second;
+        V3Tap tp;
+        tp.c = kv.second; tp.pad = 0;
+        tp.off = (k.plane * D + k.d) * t.wRow + t.wPad - k.o;
+        if (k.kind == 0) {
+            if (t.nTaps >= kV3MaxTaps) { out.why = "too many stencil taps"; return; }
+            t.hot.taps[t.nTaps++] = tp;
+        } else {
+            if (t.nSTaps >= kV3MaxSTaps) { out.why = "too many S stencil taps"; return; }
+            t.hot.staps[t.nSTaps++] = tp;
+        }
+        // what the tap adds at (kind, target, i, j, plane)
         for (int tg = 0; tg < N; ++tg) {
-            const int i = tg - tp.o, j = i - tp.d;
+            const int i = tg - k.o, j = i - k.d;
             if (i < 0 || i >= N || j < 0) continue;
-            if (tp.c0 != 0.0) have[{0, tg, i, j, 0}] += tp.c0 * ht.m[i];
-            if (tp.c1 != 0.0) have[{0, tg, i, j, 1}] += tp.c1 * ht.m[i];
-            if (tp.s1 != 0.0) have[{1, tg, i, j, 1}] += tp.s1 * ht.m[i];
+            have[{k.kind, tg, i, j, k.plane}] += kv.second * ht.m[i];
         }
     }
-    std::map<std::pair<int, int>, std::vector<V3Exc>> excBy;   // (kind, target)
+    // residuals against the table -> exception entries (coefficient per unit W = m_i n_i n_j K)
+    std::vector<V3Exc> excs;
     auto residual = [&](const std::tuple<int, int, int, int, int> &key, double w, double h) {
-        const int i = std::get<2>(key);
+        const int i = std::get<2>(key), j = std::get<3>(key), plane = std::get<4>(key);
         // coefficients are O(m_i): a difference of 1e-12 m_i is 1e-12 of the pair's own mass flux (the tables'
         // own rounding, e.g. of eps = (m_u - m) / (m_u - m_l), is of that size where eps is small)
         if (std::fabs(w - h) <= 1e-12 * ht.m[i]) return;
         V3Exc x;
-        x.coef = w - h; x.i = i; x.j = std::get<3>(key); x.plane = std::get<4>(key); x.pad = 0;
-        excBy[{std::get<0>(key), std::get<1>(key)}].push_back(x);
+        x.c = (w - h) / ht.m[i];
+        x.off = (short)((plane * D + (i - j)) * t.wRow + t.wPad + i);
+        x.kind = (short)std::get<0>(key); x.t = (short)std::get<1>(key); x.pad = 0;
+        excs.push_back(x);
     };
     for (auto &kv : want) {
         auto it = have.find(kv.first);
@@ -99,33 +106,34 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
     }
     for (auto &kv : have)
         if (!want.count(kv.first)) residual(kv.first, 0.0, kv.second);
-    if (excBy.size() > 8) {
-        out.why = "too many targets with stencil exceptions:";
-        for (auto &kv : excBy) out.why += " " + std::to_string(kv.first.first) + "/" + std::to_string(kv.first.second) + "x" + std::to_string(kv.second.size());
-        return;
+    if ((int)excs.size() > kV3MaxExc) { out.why = "too many stencil exceptions (" + std::to_string(excs.size()) + ")"; return; }
+    std::stable_sort(excs.begin(), excs.end(), [](const V3Exc &x, const V3Exc &y) {
+        return x.kind != y.kind ? x.kind < y.kind : x.t < y.t;
+    });
+    t.nExc = (int)excs.size();
+    for (int q = 0; q < t.nExc; ++q) t.hot.exc[q] = excs[q];
+    // the kernel walks taps in batches of 8: pad with entries that add nothing
+    while (t.nTaps & 7) {
+        if (t.nTaps >= kV3MaxTaps) { out.why = "too many stencil taps"; return; }
+        V3Tap z; z.c = 0.0; z.off = t.wPad; z.pad = 0;
+        t.hot.taps[t.nTaps++] = z;
     }
+    // exception entries by target: one warp sums the (at most 32) entries of a target with a fixed shuffle tree
     t.nExcT = 0;
-    for (auto &kv : excBy) {
-        V3ExcTarget &x = t.excT[t.nExcT++];
-        x.kind = (short)kv.first.first; x.t = (short)kv.first.second;
-        x.e0 = (short)out.exc.size();
-        out.exc.insert(out.exc.end(), kv.second.begin(), kv.second.end());
-        x.e1 = (short)out.exc.size();
+    for (int q = 0; q < kV3MaxExcT; ++q) { t.hot.excT[q].t = -1; t.hot.excT[q].kind = 0; t.hot.excT[q].e0 = t.hot.excT[q].e1 = 0; }
+    for (int q = 0; q < t.nExc;) {
+        int e = q;
+        while (e < t.nExc && t.hot.exc[e].kind == t.hot.exc[q].kind && t.hot.exc[e].t == t.hot.exc[q].t) ++e;
+        if (t.nExcT >= kV3MaxExcT || e - q > 32) { out.why = "too many stencil exception targets"; return; }
+        V3ExcTarget &x = t.hot.excT[t.nExcT++];
+        x.t = t.hot.exc[q].t; x.kind = t.hot.exc[q].kind; x.e0 = (short)q; x.e1 = (short)e;
+        q = e;
     }
-    t.nTaps = 0;
-    for (auto &kv : tapmap) t.taps[t.nTaps++] = kv.second;     // sorted by (d, o)
 
     // ------------------------------------------------------------------ column chunks -> warps
-    // tensor-memory columns already taken in each quarter: per-bin constants of the two combine groups
-    if (2 * nb > kV3Warps) { out.why = "too many bins for the two combine groups"; return; }
-    int used[4] = {0, 0, 0, 0};
-    for (int w = 0; w < kV3Warps; ++w) {
-        t.bincCol[w] = -1;
-        if (w < nb) { t.bincCol[w] = (short)used[w & 3]; used[w & 3] += 16; }
-        else if (w < 2 * nb) { t.bincCol[w] = (short)used[w & 3]; used[w & 3] += 2; }
-    }
+    if (3 * nb > kV3Warps) { out.why = "too many bins for the three combine groups"; return; }
     int cap[4];
-    for (int q = 0; q < 4; ++q) cap[q] = (512 - used[q]) / 32;
+    for (int q = 0; q < 4; ++q) cap[q] = 512 / 32;
     // diagonal blocks: folded row pairs
     double diagCost[kV3MaxBlk];
     for (int c = 0; c < nb; ++c) {
@@ -140,10 +148,10 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
             for (size_t q = 0; q < left.size(); ++q)
                 if (left[q] + 1 <= 32 - (rA + 1)) { rB = left[q]; left.erase(left.begin() + q); break; }
             if (nf >= kV3MaxFold) { out.why = "diagonal block needs too many folded rows"; return; }
-            t.foldA[c][nf] = (unsigned char)rA; t.foldB[c][nf] = (unsigned char)rB;
+            t.hot.foldA[c][nf] = (unsigned char)rA; t.hot.foldB[c][nf] = (unsigned char)rB;
             ++nf;
         }
-        t.nFold[c] = (short)nf;
+        t.hot.nFold[c] = (short)nf;
         diagCost[c] = kCBuildFold * nf + kCBuildDiagCopy * ((R + 7) / 8) / 4.0;
     }
     struct Chunk { int c, k, rows; };
@@ -190,76 +198,50 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
         }
     }
     // runs, tensor-memory columns, column partial slots (contiguous per column block)
-    int tcolNext[4];
-    for (int q = 0; q < 4; ++q) tcolNext[q] = used[q];
+    std::vector<std::vector<V3ColRun>> cr(kV3Warps);
+    int tcolNext[4] = {0, 0, 0, 0};
     for (int w = 0; w < kV3Warps; ++w) {
-        int nr = 0;
         for (int c = 0; c < nb; ++c)
             if (diagWarp[c] == w) {
-                if (nr >= kV3ColRuns) { out.why = "too many column runs on a warp"; return; }
                 const int n = (std::min(32, N - 32 * c) + 7) / 8;
-                V3ColRun &r = t.col[w][nr++];
-                r.c = (short)c; r.k0 = 0; r.n = (short)n; r.diag = 1;
-                r.tcol = (short)tcolNext[w & 3];
+                cr[w].push_back({c, 0, n, tcolNext[w & 3], 0, 1});
                 tcolNext[w & 3] += 32 * n;
             }
         std::sort(mine[w].begin(), mine[w].end(), [](const Chunk &x, const Chunk &y) {
             return x.c != y.c ? x.c < y.c : x.k < y.k;
         });
-        for (size_t q = 0; q < mine[w].size(); ++q) {
-            const Chunk &ch = mine[w][q];
-            if (nr > 0 && !t.col[w][nr - 1].diag && t.col[w][nr - 1].c == ch.c &&
-                t.col[w][nr - 1].k0 + t.col[w][nr - 1].n == ch.k) {
-                t.col[w][nr - 1].n++;
-            } else {
-                if (nr >= kV3ColRuns) { out.why = "too many column runs on a warp"; return; }
-                V3ColRun &r = t.col[w][nr++];
-                r.c = (short)ch.c; r.k0 = (short)ch.k; r.n = 1; r.diag = 0;
-                r.tcol = (short)tcolNext[w & 3];
-            }
+        for (const Chunk &ch : mine[w]) {
+            if (!cr[w].empty() && !cr[w].back().diag && cr[w].back().c == ch.c && cr[w].back().k0 + cr[w].back().n == ch.k)
+                cr[w].back().n++;
+            else
+                cr[w].push_back({ch.c, ch.k, 1, tcolNext[w & 3], 0, 0});
             tcolNext[w & 3] += 32;
         }
+        if ((int)cr[w].size() > kV3ColRuns) { out.why = "too many column runs on a warp"; return; }
     }
     for (int q = 0; q < 4; ++q)
         if (tcolNext[q] > 512) { out.why = "column copy exceeds tensor memory"; return; }
     {
         int slot = 0;
         for (int c = 0; c < nb; ++c) {
-            t.cpBase[c] = slot;
+            t.hot.cpBase[c] = slot;
             for (int w = 0; w < kV3Warps; ++w)
-                for (int r = 0; r < kV3ColRuns; ++r)
-                    if (t.col[w][r].n > 0 && t.col[w][r].c == c) t.col[w][r].slot = (short)slot++;
-            t.cpCnt[c] = slot - t.cpBase[c];
+                for (V3ColRun &r : cr[w])
+                    if (r.c == c) r.slot = slot++;
+            t.hot.cpCnt[c] = slot - t.hot.cpBase[c];
         }
         t.nColSlots = slot;
+        if (slot > 32) { out.why = "too many column partial slots"; return; }
     }
+    for (int w = 0; w < kV3Warps; ++w)
+        for (size_t q = 0; q < cr[w].size(); ++q)
+            t.col[w][q] = v3_pack_col(cr[w][q].c, cr[w][q].k0, cr[w][q].n, cr[w][q].tcol, cr[w][q].slot, cr[w][q].diag);
 
-    // ------------------------------------------------------------------ evaluation: band taps and row columns
+    // ------------------------------------------------------------------ evaluation: row columns
     double pre[kV3Warps];
     for (int w = 0; w < kV3Warps; ++w) {
-        pre[w] = w < nb ? kCProlPiece : 0.0;
-        for (int r = 0; r < kV3ColRuns; ++r)
-            if (t.col[w][r].n > 0) pre[w] += kCColRun + kCColChunk * t.col[w][r].n;
-        t.bandBlk[w] = -1; t.bandT0[w] = t.bandT1[w] = t.bandSlot[w] = 0;
-    }
-    {
-        // two band tasks per target block (halves of the tap list), each to the least loaded free warp
-        const int half = (t.nTaps + 1) / 2;
-        for (int g = 0; g < nb; ++g)
-            for (int h = 0; h < 2; ++h) {
-                int best = -1;
-                for (int w = 0; w < kV3Warps; ++w)
-                    if (t.bandBlk[w] < 0 && (best < 0 || pre[w] < pre[best])) best = w;
-                if (best < 0) { out.why = "no warp left for a band task"; return; }
-                t.bandBlk[best] = (short)g;
-                t.bandT0[best] = (short)(h ? half : 0); t.bandT1[best] = (short)(h ? t.nTaps : half);
-                t.bandSlot[best] = (short)h;
-                double cst = kCBandTask + kCTap * (t.bandT1[best] - t.bandT0[best]);
-                if (h == 0)
-                    for (int x = 0; x < t.nExcT; ++x)
-                        if (t.excT[x].t / 32 == g) cst += kCExcTarget;
-                pre[best] += cst;
-            }
+        pre[w] = w < nb ? kCProlPiece + kCStage : 0.0;
+        for (const V3ColRun &r : cr[w]) pre[w] += kCColRun + kCColChunk * r.n;
     }
     struct Col { int b, j; double cost; };
     std::vector<Col> cols;
@@ -269,76 +251,73 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
         for (int i = 32 * b; i < std::min(N, 32 * b + 32); ++i) {
             cmin = std::min(cmin, ht.n_bulk[i]); cmax = std::max(cmax, ht.n_bulk[i]);
         }
-        t.cmin[b] = cmin;
+        t.hot.cmin[b] = cmin;
         for (int j = 0; j < cmax; ++j) {
             cols.push_back({b, j, j < cmin ? kCRowRect : kCRowRag});
             rowTotal += cols.back().cost;
         }
     }
     {
-        double sumPre = 0.0;
-        for (int w = 0; w < kV3Warps; ++w) sumPre += pre[w];
-        // water level: warps whose preload already exceeds it take no row work
-        double level = (sumPre + rowTotal) / kV3Warps;
-        for (int it = 0; it < 8; ++it) {
-            double room = 0.0; int n = 0;
-            for (int w = 0; w < kV3Warps; ++w)
-                if (pre[w] < level) { room += level - pre[w]; ++n; }
-            if (n == 0) break;
-            level += (rowTotal + kCRowRun * n - room) / n;
+        // water level L with sum_w max(0, L - pre[w] - run overhead) = row work (bisection)
+        double lo = 0.0, hi = 0.0;
+        for (int w = 0; w < kV3Warps; ++w) hi = std::max(hi, pre[w]);
+        hi += rowTotal + kCRowRun;
+        for (int it = 0; it < 60; ++it) {
+            const double L = 0.5 * (lo + hi);
+            double room = 0.0;
+            for (int w = 0; w < kV3Warps; ++w) room += std::max(0.0, L - pre[w] - kCRowRun);
+            (room < rowTotal ? lo : hi) = L;
         }
+        const double level = hi;
         size_t next = 0;
-        int slotCount = 0;
         std::vector<std::vector<V3RowRun>> rr(kV3Warps);
+        auto left_in_block = [&](size_t q) {            // columns of cols[q]'s block from q on
+            size_t e = q;
+            while (e < cols.size() && cols[e].b == cols[q].b) ++e;
+            return (int)(e - q);
+        };
         auto give = [&](int w, double budget) {
-            while (next < cols.size() && budget > 0.0) {
-                if (rr[w].empty() || rr[w].back().b != cols[next].b) {
+            while (next < cols.size()) {
+                const bool same = !rr[w].empty() && rr[w].back().b == cols[next].b;
+                if (budget <= 0.0 && !(same && left_in_block(next) <= 5)) break;    // a short block tail stays with its run
+                if (!same) {
                     if ((int)rr[w].size() >= kV3RowRuns) return;
-                    V3RowRun r;
-                    r.b = (short)cols[next].b; r.ja = r.jb = (short)cols[next].j; r.slot = 0;
-                    rr[w].push_back(r);
-                    budget -= kCRowRun;
+                    if (budget < 8.0 * cols[next].cost + (rr[w].empty() ? 0.0 : kCRowRun)) return;   // not worth a run
+                    rr[w].push_back({cols[next].b, cols[next].j, cols[next].j, 0});
+                    if (rr[w].size() > 1) budget -= kCRowRun;
                 }
                 rr[w].back().jb++;
                 budget -= cols[next].cost;
                 ++next;
             }
         };
-        for (int w = 0; w < kV3Warps; ++w) give(w, level - pre[w]);
+        for (int w = 0; w < kV3Warps; ++w) give(w, level - pre[w] - kCRowRun);
         for (int w = kV3Warps - 1; w >= 0 && next < cols.size(); --w) give(w, 1e30);   // rounding leftovers
         if (next < cols.size()) { out.why = "row pass does not fit the run lists"; return; }
+        int slotCount = 0;
         for (int b = 0; b < nb; ++b) {
-            t.rpBase[b] = slotCount;
+            t.hot.rpBase[b] = slotCount;
             for (int w = 0; w < kV3Warps; ++w)
                 for (V3RowRun &r : rr[w])
-                    if (r.b == b && r.jb > r.ja) r.slot = (short)slotCount++;
-            t.rpCnt[b] = slotCount - t.rpBase[b];
+                    if (r.b == b && r.jb > r.ja) r.slot = slotCount++;
+            t.hot.rpCnt[b] = slotCount - t.hot.rpBase[b];
         }
         t.nRowSlots = slotCount;
+        if (slotCount > 32) { out.why = "too many row partial slots"; return; }
         for (int w = 0; w < kV3Warps; ++w)
-            for (size_t q = 0; q < rr[w].size(); ++q) t.row[w][q] = rr[w][q];
+            for (size_t q = 0; q < rr[w].size(); ++q)
+                if (rr[w][q].jb > rr[w][q].ja) t.row[w][q] = v3_pack_row(rr[w][q].b, rr[w][q].ja, rr[w][q].jb, rr[w][q].slot);
     }
 
     // ------------------------------------------------------------------ shared-memory layout (bytes)
     {
-        int q = 0;
-        auto take = [&](int bytes) { const int o = q; q += (bytes + 15) & ~15; return o; };
-        t.oYY = take(16 * (Np + 2 * kV3Pad));
-        t.oNN = take(8 * (Np + 2 * kV3Pad + 8));
-        t.oDTAB = take(16 * Np);
-        t.oEXPT = take(8 * 64);
-        t.oRED = take(8 * 128);
-        t.oBAND = take(8 * 4 * Np);                 // [slot][kind][Np]
-        t.oGK = take(8 * 2 * Np);                   // G_k, scanned suffix
-        t.oNBULK = take(8 * Np);                   // int2 per bin: n_bulk | iS << 9, jS_lo | jS_hi << 16
-        t.oUNION = q;
-        const int roles = 8 * 19 * Np;
-        t.oCOLP = t.oUNION;
-        t.oROWP = t.oCOLP + 512 * t.nColSlots;
-        const int parts = 512 * t.nColSlots + 1024 * t.nRowSlots;
-        q += (std::max(roles, parts) + 15) & ~15;
-        t.oK = q;
-        t.smemBytes = q + 16 * P;
+        const int wst = 8 * 2 * D * t.wRow;
+        t.oWST = kV3oUNION;
+        t.oCOLP = t.oWST + ((wst + 15) & ~15);
+        t.oROWP = t.oCOLP + kV3ColSlotBytes * t.nColSlots;
+        const int evalBytes = t.oROWP + kV3RowSlotBytes * t.nRowSlots - kV3oUNION;
+        t.oK = kV3oUNION + ((std::max(kV3BuildUnionBytes, evalBytes) + 15) & ~15);
+        t.smemBytes = t.oK + 16 * P;
     }
     if (t.smemBytes > smem_optin) { out.why = "kernel of a cell does not fit shared memory"; return; }
     t.on = 1;
@@ -347,7 +326,7 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
 void v3_check(const HostTables &ht, const V3Host &v, long long bad[6])
 {
     const V3Tables &t = v.t;
-    const int N = ht.N, nb = t.nb, Np = 32 * nb;
+    const int N = ht.N, nb = t.nb, D = t.bandD;
     std::vector<int> built((size_t)N * N, 0), rowc((size_t)N * N, 0), colc((size_t)N * N, 0);
     std::vector<int> tmap(4 * 512, 0), cslot(std::max(1, t.nColSlots), 0), rslot(std::max(1, t.nRowSlots), 0);
     auto claim = [&](int q, int col, int n) {
@@ -356,22 +335,21 @@ void v3_check(const HostTables &ht, const V3Host &v, long long bad[6])
         }
     };
     for (int w = 0; w < kV3Warps; ++w) {
-        if (w < nb) claim(w & 3, t.bincCol[w], 16);
-        else if (w < 2 * nb) claim(w & 3, t.bincCol[w], 2);
         for (int r = 0; r < kV3ColRuns; ++r) {
-            const V3ColRun &run = t.col[w][r];
-            if (run.n == 0) continue;
+            if (!t.col[w][r]) continue;
+            const V3ColRun run = v3_unpack_col(t.col[w][r]);          // the decode the device uses
+            if (run.n == 0) { ++bad[3]; continue; }
             claim(w & 3, run.tcol, 32 * run.n);
-            if (run.slot < t.cpBase[run.c] || run.slot >= t.cpBase[run.c] + t.cpCnt[run.c] || cslot[run.slot]++) ++bad[3];
+            if (run.slot < t.hot.cpBase[run.c] || run.slot >= t.hot.cpBase[run.c] + t.hot.cpCnt[run.c] || cslot[run.slot]++) ++bad[3];
             // column pass: rows of the chunks x the 32 columns of the block
             for (int i = 32 * run.c + 8 * run.k0; i < std::min(N, 32 * run.c + 8 * (run.k0 + run.n)); ++i)
                 for (int j = 32 * run.c; j < std::min(N, 32 * run.c + 32); ++j)
                     if (i >= j) colc[(size_t)i * N + j]++;
             if (run.diag) {
                 if (run.k0 != 0 || run.n != (std::min(32, N - 32 * run.c) + 7) / 8) ++bad[0];
-                for (int fi = 0; fi < t.nFold[run.c]; ++fi)
+                for (int fi = 0; fi < t.hot.nFold[run.c]; ++fi)
                     for (int lane = 0; lane < 32; ++lane) {
-                        const int rA = t.foldA[run.c][fi], rB = t.foldB[run.c][fi];
+                        const int rA = t.hot.foldA[run.c][fi], rB = t.hot.foldB[run.c][fi];
                         int r2, q;
                         if (lane <= rA) { r2 = rA; q = lane; }
                         else if (rB != 0xff && lane - rA - 1 <= rB) { r2 = rB; q = lane - rA - 1; }
@@ -390,12 +368,13 @@ void v3_check(const HostTables &ht, const V3Host &v, long long bad[6])
             }
         }
         for (int r = 0; r < kV3RowRuns; ++r) {
-            const V3RowRun &run = t.row[w][r];
-            if (run.jb == run.ja) continue;
-            if (run.slot < t.rpBase[run.b] || run.slot >= t.rpBase[run.b] + t.rpCnt[run.b] || rslot[run.slot]++) ++bad[3];
+            if (!t.row[w][r]) continue;
+            const V3RowRun run = v3_unpack_row(t.row[w][r]);
+            if (run.jb <= run.ja) { ++bad[3]; continue; }
+            if (run.slot < t.hot.rpBase[run.b] || run.slot >= t.hot.rpBase[run.b] + t.hot.rpCnt[run.b] || rslot[run.slot]++) ++bad[3];
             for (int i = 32 * run.b; i < std::min(N, 32 * run.b + 32); ++i)
                 for (int j = run.ja; j < run.jb; ++j) {
-                    if (j < t.cmin[run.b] && j >= ht.n_bulk[i]) ++bad[1];      // the rectangle must be bulk
+                    if (j < t.hot.cmin[run.b] && j >= ht.n_bulk[i]) ++bad[1];      // the rectangle must be bulk
                     if (j < ht.n_bulk[i]) rowc[(size_t)i * N + j]++;
                 }
         }
@@ -408,20 +387,14 @@ void v3_check(const HostTables &ht, const V3Host &v, long long bad[6])
             bad[1] += rowc[(size_t)i * N + j] != (j < ht.n_bulk[i] ? 1 : 0);
             bad[2] += colc[(size_t)i * N + j] != 1;
         }
-    if (t.oROWP + 1024 * t.nRowSlots > t.oK || t.oUNION + 8 * 19 * Np > t.oK) ++bad[3];
-    // band tasks: both halves of every block, taps covered once
-    for (int g = 0; g < nb; ++g) {
-        std::vector<int> cov(std::max(1, t.nTaps), 0);
-        int slots = 0;
-        for (int w = 0; w < kV3Warps; ++w)
-            if (t.bandBlk[w] == g) {
-                slots |= 1 << t.bandSlot[w];
-                for (int q = t.bandT0[w]; q < t.bandT1[w]; ++q) cov[q]++;
-            }
-        if (slots != 3) ++bad[5];
-        for (int q = 0; q < t.nTaps; ++q) bad[5] += cov[q] != 1;
-    }
-    // stencil + exceptions against the gather entries on pseudo-random n and K
+    // layout: stage, slots and role vectors below the row copy; the band pairs are all inside the stage
+    if (t.oWST != kV3oUNION || t.oCOLP < t.oWST + 8 * 2 * D * t.wRow || t.oROWP != t.oCOLP + kV3ColSlotBytes * t.nColSlots ||
+        t.oROWP + kV3RowSlotBytes * t.nRowSlots > t.oK || kV3oUNION + kV3BuildUnionBytes > t.oK ||
+        t.smemBytes != t.oK + 16 * t.P) ++bad[3];
+    for (int i = 0; i < N; ++i)
+        for (int j = ht.n_bulk[i]; j <= i; ++j)
+            if (i - j >= D) ++bad[4];
+    // stencil + exceptions against the gather entries on pseudo-random n and K, through the stage layout
     {
         std::vector<double> n(N), Kc((size_t)N * N), Kf((size_t)N * N);
         unsigned long long sd = 88172645463325252ull;
@@ -433,21 +406,33 @@ void v3_check(const HostTables &ht, const V3Host &v, long long bad[6])
             const double x = e.coef * n[e.i] * n[e.j] * (e.plane ? Kf : Kc)[(size_t)e.i * N + e.j];
             ref[e.target] += x; refAbs[e.target] += std::fabs(x);
         }
-        for (int q = 0; q < t.nTaps; ++q)
-            for (int tg = 0; tg < N; ++tg) {
-                const int i = tg - t.taps[q].o, j = i - t.taps[q].d;
-                if (i < 0 || i >= N || j < 0) continue;
-                const double w = ht.m[i] * n[i] * n[j];
-                got[tg] += w * (t.taps[q].c0 * Kc[(size_t)i * N + j] + t.taps[q].c1 * Kf[(size_t)i * N + j]);
-                got[N + tg] += w * t.taps[q].s1 * Kf[(size_t)i * N + j];
-            }
-        for (int x = 0; x < t.nExcT; ++x)
-            for (int e = t.excT[x].e0; e < t.excT[x].e1; ++e) {
-                const V3Exc &ex = v.exc[e];
-                got[t.excT[x].kind * N + t.excT[x].t] += ex.coef * n[ex.i] * n[ex.j] * (ex.plane ? Kf : Kc)[(size_t)ex.i * N + ex.j];
-            }
+        std::vector<double> W((size_t)2 * D * t.wRow, 0.0);
+        for (int p = 0; p < 2; ++p)
+            for (int d = 0; d < D; ++d)
+                for (int i = d; i < N; ++i)
+                    W[(size_t)(p * D + d) * t.wRow + t.wPad + i] = ht.m[i] * n[i] * n[i - d] * (p ? Kf : Kc)[(size_t)i * N + i - d];
+        auto at = [&](long idx) -> double {
+            if (idx < 0 || idx >= (long)W.size()) { ++bad[4]; return 0.0; }
+            return W[(size_t)idx];
+        };
+        for (int tg = 0; tg < N; ++tg) {
+            for (int q = 0; q < t.nTaps; ++q) got[tg] += t.hot.taps[q].c * at((long)t.hot.taps[q].off + tg);
+            for (int q = 0; q < t.nSTaps; ++q) got[N + tg] += t.hot.staps[q].c * at((long)t.hot.staps[q].off + tg);
+        }
+        for (int q = 0; q < t.nExc; ++q) {
+            if (t.hot.exc[q].t < 0 || t.hot.exc[q].t >= N) { ++bad[4]; continue; }
+            got[t.hot.exc[q].kind * N + t.hot.exc[q].t] += t.hot.exc[q].c * at(t.hot.exc[q].off);
+        }
         for (int q = 0; q < 2 * N; ++q)
             if (std::fabs(got[q] - ref[q]) > 1e-12 * refAbs[q]) ++bad[4];
+        // every exception entry inside exactly one target range of its own (kind, t)
+        std::vector<int> cov(std::max(1, t.nExc), 0);
+        for (int x = 0; x < t.nExcT; ++x)
+            for (int e = t.hot.excT[x].e0; e < t.hot.excT[x].e1; ++e) {
+                if (e < 0 || e >= t.nExc || t.hot.exc[e].t != t.hot.excT[x].t || t.hot.exc[e].kind != t.hot.excT[x].kind) { ++bad[4]; continue; }
+                cov[e]++;
+            }
+        for (int e = 0; e < t.nExc; ++e) bad[4] += cov[e] != 1;
     }
 }
 
