@@ -73,7 +73,6 @@ struct cudisc_grid_s {
     double *trial_rho, *trial_k, *trial_err, *d_log;   // cudisc_coag_integrate (lazy, all or nothing)
     CtrlState *d_ctrl, *h_ctrl;                        // controller state: device, pinned host mirror
     int log_cap;
-    long long *prof;    // CUDISC_PROF builds only
     int num_sms, smem_optin, grid_ctas, Psm, smem_bytes;
     bool fast;          // cudisc_coag_step / rates_otf run on the tensor-memory kernel
     int fast_ctas;
@@ -408,12 +407,10 @@ int run(cudisc_grid g, int mode, GasArgs ga, StepArgs sa, cudisc_stream stream, 
     }
     sa.Psm = g->Psm;
     sa.kslab = g->kslab;
-    sa.prof = g->prof;
     LaunchCfg lc{std::min(g->grid_ctas, std::max(1, sa.C)), g->smem_bytes, g->smem_optin};
     cudaError_t e;
     if (g->fast && (mode == MODE_OTF || mode == MODE_STEP) && !ga.hd && !ga.vphi) {
         LaunchCfg lf{std::min(g->fast_ctas, std::max(1, sa.C)), g->bins->v3.smemBytes, g->smem_optin};
-        sa.Psm = getenv("V3_DEBUG") ? atoi(getenv("V3_DEBUG")) : 0;
         e = launch_v3(mode, lf, g->bins->dt, g->bins->v3, ga, sa, (cudaStream_t)stream);
     } else {
         e = launch_cells(mode, lc, g->bins->dt, ga, sa, (cudaStream_t)stream);
@@ -671,7 +668,7 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
     g->gas_bound = false; g->fsal_valid = false;
     g->fsal_rho = g->fsal_K = nullptr;
     g->k_fsal = nullptr; g->kslab = nullptr;
-    g->stage_rho = nullptr; g->stage_err = nullptr; g->prof = nullptr;
+    g->stage_rho = nullptr; g->stage_err = nullptr;
     g->pipe[0] = g->pipe[1] = nullptr;
     g->pipe_ev[0] = g->pipe_ev[1] = g->pipe_ev[2] = nullptr;
     g->trial_rho = g->trial_k = g->trial_err = g->d_log = nullptr;
@@ -702,25 +699,10 @@ int cudisc_grid_create(int n_r, int n_z, cudisc_bins b, cudisc_grid *out)
         delete g;
         return cuda_fail(e, "cudaMalloc(grid)");
     }
-#ifdef CUDISC_PROF
-    cudaMalloc((void **)&g->prof, (size_t)g->grid_ctas * 48 * sizeof(long long));
-    cudaMemset(g->prof, 0, (size_t)g->grid_ctas * 48 * sizeof(long long));
-#endif
     *out = g;
     return CUDISC_OK;
 }
 
-#ifdef CUDISC_PROF
-/* working builds only: phase cycle counters of CTA 0..n-1, 16 per CTA; resets them */
-int cudisc_debug_prof(cudisc_grid g, long long *out_host, int n_ctas)
-{
-    cudaDeviceSynchronize();
-    n_ctas = std::min(n_ctas, g->grid_ctas);
-    cudaMemcpy(out_host, g->prof, (size_t)n_ctas * 48 * sizeof(long long), cudaMemcpyDeviceToHost);
-    cudaMemset(g->prof, 0, (size_t)g->grid_ctas * 48 * sizeof(long long));
-    return n_ctas;
-}
-#endif
 
 int cudisc_grid_bind_gas(cudisc_grid g, const cudisc_gas_state *gs)
 {
@@ -749,7 +731,6 @@ int cudisc_grid_destroy(cudisc_grid g)
     if (g->stage_err) cudaFree(g->stage_err);
     for (int q = 0; q < 2; ++q) if (g->pipe[q]) cudaStreamDestroy(g->pipe[q]);
     for (int q = 0; q < 3; ++q) if (g->pipe_ev[q]) cudaEventDestroy(g->pipe_ev[q]);
-    if (g->prof) cudaFree(g->prof);
     if (g->trial_rho) cudaFree(g->trial_rho);
     if (g->trial_k) cudaFree(g->trial_k);
     if (g->trial_err) cudaFree(g->trial_err);

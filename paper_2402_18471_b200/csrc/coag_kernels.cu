@@ -95,11 +95,10 @@ __device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, c
 // Three block barriers; every partial sum has its own slot and every combination a fixed order.
 template <int NT, bool SLAB>
 __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
-                                             double y, int tid, uint32_t tbase, long long *sa_prof,
+                                             double y, int tid, uint32_t tbase,
                                              bool pre, const CellGas &nx, double mu, double sigma_mol,
                                              RoleVals &rv)
 {
-    PROF_T(tp0);
     const int N = tb.N, Np = tb.Np;
     const int lane = tid & 31, warp = tid >> 5;
     const int k = tid;
@@ -118,8 +117,6 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     }
     if (tid == 0) { s.CTR[1] = NT / 32; s.CTR[2] = 0; }
     __syncthreads();
-    PROF_ADD(2, tp0);
-    PROF_T(tpA);
 
     // per-bin values of the NEXT cell (inputs were fetched an evaluation ago): the bin-owning warps
     // compute them here, in registers, while the other warps start on the items
@@ -128,7 +125,6 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     // ---- phase A: band gathers from tensor memory (tasks fixed per warp: a warp only reaches the
     //      tensor-memory lanes of its quarter), then row sums, column sums (and, without
     //      tensor-memory tables, band gathers) pulled by warps
-#ifndef CUDISC_NOBAND
     if (tb.bandTmem && !tb.bandD) {
 #pragma unroll 1
         for (int q = 0; q < 2; ++q) {
@@ -157,10 +153,6 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
             if (t < 2 * N) (((task >> 30) & 1) ? s.BANDV2 : s.BANDV)[t] = acc0 + acc1;
         }
     }
-#endif
-#ifdef CUDISC_NOBAND
-    if (false)
-#endif
     // band gathers from the staged products (tensor-memory coefficients and stage indices): run by the
     // owning warp after its first item, when the (short, first-claimed) W items are done
     auto band_from_stage = [&]() {
@@ -290,10 +282,7 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         if (!band_done) { band_from_stage(); band_done = true; }
     }
     if (!band_done) band_from_stage();
-    PROF_ADD(3, tpA);
     __syncthreads();
-    PROF_ADD(4, tpA);
-    PROF_T(tpB);
 
     // ---- phase B: combine partials in fixed order.  Two warp groups work side by side:
     //   group R (thread k, bin k)            row partials -> deposits into bins k-1, k, k+1
@@ -380,7 +369,6 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
         d = fma(-y, s.NN[k], d);
         d = fma(s.BINC[BC_FA * Np + k], suf, d);
     }
-    PROF_ADD(5, tpB);
     return d;
 }
 
@@ -457,8 +445,6 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
     __syncthreads();
     if (use_tmem) tmem_fence_after();
 
-    long long *sa_prof = sa.prof ? sa.prof + 48 * (size_t)blockIdx.x : nullptr;
-    (void)sa_prof;
     const int k = tid;
     const bool live = k < N;
 
@@ -483,7 +469,6 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
     bool rv_valid = false;       // rv holds the next cell's values (computed during the last evaluation)
 
     for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
-        PROF_T(tc0);
         const size_t row = (size_t)cell * N;
 
         // ---------------- K store for this cell
@@ -518,7 +503,6 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
             if (tid == 0) { s.CTR[0] = NT / 32; s.RED[95] = rv.Vg2; }
             __syncthreads();
             pc.Vg2 = s.RED[95];
-            PROF_ADD(0, tc0);
         }
         // state (thread <-> bin): in flight during the build
         double y0 = 0.0, k1 = 0.0;
@@ -550,12 +534,11 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
             }
             __syncthreads();
         }
-        PROF_ADD(1, tc0);
         if (MODE == MODE_KERNEL) continue;
 
         if (MODE == MODE_RATES || MODE == MODE_OTF) {
             fetch(cell + gridDim.x);
-            const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, tbase, sa_prof, false, nx, gs.mu, gs.sigma_mol, rv);
+            const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, tbase, false, nx, gs.mu, gs.sigma_mol, rv);
             if (live) sa.out[row + k] = d;
             __syncthreads();
             continue;
@@ -564,7 +547,6 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
         // ---------------- Bogacki-Shampine 3(2), PAPER.md:478 (tableau: Bogacki & Shampine 1989)
         const double h = sa.dt;
         double k2 = 0.0, k3 = 0.0, k4 = 0.0, yn = y0;
-        PROF_T(tst);
 #pragma unroll 1
         for (int st = sa.have_k1 ? 1 : 0; st < 4; ++st) {
             double ys = y0;
@@ -576,7 +558,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
                 ys = yn;
             }
             const bool pre = MODE == MODE_STEP && st == 3 && cell + (int)gridDim.x < sa.C;
-            const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, tbase, sa_prof, pre, nx, gs.mu,
+            const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, tbase, pre, nx, gs.mu,
                                                   gs.sigma_mol, rv);
             if (st == 3) rv_valid = pre;
             if (st == 0) k1 = d;
@@ -585,8 +567,6 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
             if (st == 3) k4 = d;
         }
 
-        PROF_ADD(8, tst);
-        PROF_T(ttail);
         // error norm (R10) and write-back
         const double atol = sa.atol_factor * block_sum<NT>(y0, s.RED + 48, tid);
         double emax = 0.0;
@@ -599,8 +579,6 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
         }
         emax = block_nanmax<NT>(emax, s.RED + 64, tid);
         if (tid == 0) sa.err[cell] = emax;
-        PROF_ADD(7, ttail);
-        PROF_ADD(6, tc0);
     }
     if (use_tmem) {
         tmem_fence_before();

@@ -38,6 +38,17 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32
                     "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
                  : "memory");
 }
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                 "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                   "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                   "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                 : "r"(taddr) : "memory");
+}
 // 8-byte asynchronous global -> shared copy (LDGSTS): inputs of a cell are staged in shared memory
 // while the build runs, without holding registers across it
 __device__ __forceinline__ void cp_async8(void *dst_smem, const void *src_gmem)
@@ -50,22 +61,6 @@ __device__ __forceinline__ double u2d(uint32_t lo, uint32_t hi) { return __hiloi
 __device__ __forceinline__ uint32_t dlo(double x) { return (uint32_t)__double2loint(x); }
 __device__ __forceinline__ uint32_t dhi(double x) { return (uint32_t)__double2hiint(x); }
 
-#ifdef CUDISC_PROF
-// clock64 that cannot issue before a shared-memory load issued after the barrier has returned
-__device__ __forceinline__ long long clock_after_barrier(const void *smem_word)
-{
-    long long c;
-    asm volatile("{\n .reg .pred p;\n .reg .u32 v;\n ld.volatile.shared.u32 v, [%1];\n setp.ne.u32 p, v, 0x7fc00001;\n"
-                 " mov.u64 %0, 0;\n @p mov.u64 %0, %%clock64;\n}\n"
-                 : "=l"(c) : "r"((uint32_t)__cvta_generic_to_shared(smem_word)) : "memory");
-    return c;
-}
-#define PROF_TB(var) const long long var = clock_after_barrier(f.RED())
-#define PROF_ADDB(slot, t0) do { const long long c_ = clock_after_barrier(f.RED()); if (threadIdx.x == 0) sa_prof[(slot)] += c_ - (t0); } while (0)
-#else
-#define PROF_TB(var)
-#define PROF_ADDB(slot, t0)
-#endif
 
 // ------------------------------------------------------------------------------------------ shared memory
 // Fixed arrays at compile-time offsets (coag_v3.h kV3o*): their addresses fold into the instructions.
@@ -90,8 +85,9 @@ __device__ __forceinline__ VSm v3_carve(char *base, const DevTables &tb, const V
     Smem &s = f.s;
     double *u = (double *)(base + kV3oUNION);
     s.YY = f.YY(); s.NN = f.NN();
-    s.DTAB = const_cast<double2 *>(tb.dtab);      // grid-only tables of the pair kernel: read through L1
-    s.EXPT = const_cast<double *>(tb.exptab);
+    // grid-only tables of the pair kernel: shared memory if the cell leaves room, else read through L1
+    s.DTAB = vt.oDTAB ? (double2 *)(base + vt.oDTAB) : const_cast<double2 *>(tb.dtab);
+    s.EXPT = vt.oDTAB ? (double *)(base + vt.oDTAB + 16 * vt.N) : const_cast<double *>(tb.exptab);
     s.RED = f.RED();
     s.BANDV = s.BANDV2 = nullptr; s.WST = nullptr; s.BINC = nullptr; s.BINI = f.BINI();
     s.CTR = nullptr; s.SCHED = nullptr; s.ITB = s.ITE = nullptr; s.PARTR = s.PARTC = nullptr;
@@ -194,25 +190,25 @@ __device__ __forceinline__ void v3_col_run(const V3Tables &vt, const VSm &f, con
     uint32_t ta = tq + (uint32_t)run.tcol;
     const double *nn = f.NN() + 32 * run.c + 8 * run.k0;
     double gc = 0.0, h = 0.0, gc2 = 0.0, h2 = 0.0;
-    // half a chunk (4 rows) per tcgen05.ld.x16; the next half is in flight while this one is summed
-    auto half = [&](const uint32_t (&v)[16], const double *n4) {
-        const double2 n01 = *reinterpret_cast<const double2 *>(n4);
-        const double2 n23 = *reinterpret_cast<const double2 *>(n4 + 2);
+    // one chunk (8 rows) per tcgen05.ld.x32 (tcgen05.wait::ld drains every load in flight, so a deeper
+    // pipeline of smaller loads only adds round trips)
+#pragma unroll 1
+    for (int kk = 0; kk < run.n; ++kk) {
+        uint32_t v[32];
+        tmem_ld32(ta, v);
+        const double2 n01 = *reinterpret_cast<const double2 *>(nn);
+        const double2 n23 = *reinterpret_cast<const double2 *>(nn + 2);
+        const double2 n45 = *reinterpret_cast<const double2 *>(nn + 4);
+        const double2 n67 = *reinterpret_cast<const double2 *>(nn + 6);
+        tmem_wait_ld();
         gc = fma(u2d(v[0], v[1]), n01.x, gc);      h = fma(u2d(v[2], v[3]), n01.x, h);
         gc2 = fma(u2d(v[4], v[5]), n01.y, gc2);    h2 = fma(u2d(v[6], v[7]), n01.y, h2);
         gc = fma(u2d(v[8], v[9]), n23.x, gc);      h = fma(u2d(v[10], v[11]), n23.x, h);
         gc2 = fma(u2d(v[12], v[13]), n23.y, gc2);  h2 = fma(u2d(v[14], v[15]), n23.y, h2);
-    };
-    uint32_t va[16], vb[16];
-    tmem_ld16(ta, va);
-#pragma unroll 1
-    for (int kk = 0; kk < run.n; ++kk) {
-        tmem_wait_ld();
-        tmem_ld16(ta + 16, vb);
-        half(va, nn);
-        tmem_wait_ld();
-        if (kk + 1 < run.n) tmem_ld16(ta + 32, va);
-        half(vb, nn + 4);
+        gc = fma(u2d(v[16], v[17]), n45.x, gc);    h = fma(u2d(v[18], v[19]), n45.x, h);
+        gc2 = fma(u2d(v[20], v[21]), n45.y, gc2);  h2 = fma(u2d(v[22], v[23]), n45.y, h2);
+        gc = fma(u2d(v[24], v[25]), n67.x, gc);    h = fma(u2d(v[26], v[27]), n67.x, h);
+        gc2 = fma(u2d(v[28], v[29]), n67.y, gc2);  h2 = fma(u2d(v[30], v[31]), n67.y, h2);
         ta += 32; nn += 8;
     }
     reinterpret_cast<double2 *>(f.base + vt.oCOLP)[32 * run.slot + lane] = make_double2(gc + gc2, h + h2);
@@ -282,8 +278,10 @@ __device__ __forceinline__ void v3_stage(const V3Tables &vt, const VSm &f, int i
             const double yn = yi * nn[-d];
             wc = yn * k2.x; wf = yn * k2.y;
         }
-        w[d * vt.wRow] = wc;
-        w[plane + d * vt.wRow] = wf;
+        if (i < N) {                                 // (rows of the stage hold the N bins + padding)
+            w[d * vt.wRow] = wc;
+            w[plane + d * vt.wRow] = wf;
+        }
     }
 }
 
@@ -332,15 +330,12 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
                                           double c1, double c2, double c3, int tid, uint32_t tq, int ppart,
                                           const CellGas &nx, double mu, double sigma_mol, ProlState &ps,
                                           RoleVals &rv, const uint32_t (&colw)[kV3ColRuns],
-                                          const uint32_t (&roww)[kV3RowRuns], int dbg)
+                                          const uint32_t (&roww)[kV3RowRuns])
 {
     const int N = vt.N, nb = vt.nb;
     const int lane = tid & 31, warp = tid >> 5;
     const int k = tid;
     const bool live = k < N;
-    long long *sa_prof = reinterpret_cast<long long *>(f.RED() + 96);
-    (void)sa_prof;
-    PROF_T(tp0);
 
     // ---- phase 0
     double nk = 0.0;
@@ -350,13 +345,11 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         f.YY()[k] = make_double2(y, y * c1);
     }
     __syncthreads();
-    PROF_ADDB(2, tp0);
-    PROF_TB(tpA);
 
     // ---- phase A: the bin-owning warps stage the band products of their bins and run a third of the NEXT
     //      cell's prologue (ppart 1, 2, 3; 4: all of it); then every warp its own runs
     if (warp < nb) {
-        if (!(dbg & 1)) v3_stage(vt, f, k, live ? y : 0.0);
+        v3_stage(vt, f, k, live ? y : 0.0);
         if (ppart) {
             if (ppart == 1 || ppart == 4) ps = prologue_begin(tb, nx, mu, sigma_mol, k);
             prologue_newton(ps, ppart == 4 ? 6 : 2);
@@ -368,22 +361,16 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
 #pragma unroll 1
     for (int r = 0; r < kV3ColRuns; ++r) {
         const uint32_t w = r == 0 ? colw[0] : (r == 1 ? colw[1] : (r == 2 ? colw[2] : colw[3]));
-        if (!w || (dbg & 2)) break;
+        if (!w) break;
         v3_col_run(vt, f, v3_unpack_col(w), tq, lane);
     }
 #pragma unroll 1
     for (int r = 0; r < kV3RowRuns; ++r) {
         const uint32_t w = r == 0 ? roww[0] : (r == 1 ? roww[1] : roww[2]);
-        if (!w || (dbg & 4)) break;
+        if (!w) break;
         v3_row_run(tb, vt, f, v3_unpack_row(w), lane);
     }
-    PROF_ADD(3, tpA);
-#ifdef CUDISC_PROF
-    if (lane == 0) sa_prof[16 + warp] += clock64() - tpA;     // RED[112 ..]: per-warp busy time of phase A
-#endif
     __syncthreads();
-    PROF_ADDB(4, tpA);
-    PROF_TB(tpB);
 
     // ---- phase B (combine), three groups of warps side by side:
     //   R (warp w < nb, bin 32 w + lane)      row partials -> deposits into bins k-1, k, k+1; first half of the
@@ -395,8 +382,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
     double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, up = 0.0, dn = 0.0, bandR = 0.0;
     double *wtot = f.RED(), *eUp = f.RED() + 16, *eDn = f.RED() + 32;
     const double *wst = f.WST();
-    if (dbg & 8) {
-    } else if (warp < nb) {
+    if (warp < nb) {
         const double *pp = reinterpret_cast<const double *>(f.base + vt.oROWP) + 96 * f.HOT()->rpBase[warp] + lane;
         const int np = f.HOT()->rpCnt[warp];
 #pragma unroll 4
@@ -408,7 +394,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         if (lane == 31) eUp[warp] = dp1;
         up = __shfl_up_sync(0xffffffffu, dp1, 1);
         dn = __shfl_down_sync(0xffffffffu, dm1, 1);
-        bandR = v3_taps(f, wst, k, 0, vt.nTaps >> 1);
+        bandR = v3_taps(f, wst, min(k, N - 1), 0, vt.nTaps >> 1);
     } else if (warp < 2 * nb) {
         const int g = warp - nb, kc = 32 * g + lane;
         const double2 *colp = reinterpret_cast<const double2 *>(f.base + vt.oCOLP);
@@ -425,7 +411,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         double sl = 0.0;
         {   // S stencil of l-bin kc (stage entries past the bins are 0) and its exceptions
 #pragma unroll 1
-            for (int q = 0; q < vt.nSTaps; ++q) sl = fma(f.HOT()->staps[q].c, wst[f.HOT()->staps[q].off + kc], sl);
+            for (int q = 0; q < vt.nSTaps; ++q) sl = fma(f.HOT()->staps[q].c, wst[f.HOT()->staps[q].off + min(kc, N - 1)], sl);
         }
         sl = v3_exceptions(f, wst, g, 1, lane, sl);
         if (kc < N) {
@@ -448,24 +434,13 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         }
         if (lane == 0) wtot[g] = suf;
         if (kc < N) f.YY()[kc].y = suf;
-#ifdef CUDISC_PROF
-        if (tid == 32 * nb) sa_prof[9] += clock64() - tpB;
-#endif
     } else if (warp < 3 * nb) {
-#ifdef CUDISC_PROF
-        if (tid == 64 * nb) sa_prof[13] += clock64() - tpB;
-#endif
         const int g = warp - 2 * nb, t = 32 * g + lane;
-        double da = v3_taps(f, wst, t, vt.nTaps >> 1, vt.nTaps);       // (the list is padded to a multiple of 8)
+        double da = v3_taps(f, wst, min(t, N - 1), vt.nTaps >> 1, vt.nTaps);       // (the list is padded to a multiple of 8)
         da = v3_exceptions(f, wst, g, 0, lane, da);
         f.BANDV()[t] = da;
-#ifdef CUDISC_PROF
-        if (tid == 64 * nb) sa_prof[10] += clock64() - tpB;
-#endif
     }
-    PROF_ADD(5, tpB);
     __syncthreads();
-    PROF_ADDB(7, tpB);
     if (warp >= nb) return 0.0;
 
     double d = 0.0;
@@ -481,7 +456,6 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         d = fma(-y, f.NN()[k], d);
         d = fma(c3, suf, d);
     }
-    PROF_ADD(6, tpB);
     return d;
 }
 
@@ -501,13 +475,16 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     pc.Vg2 = 0.0;
     const int k = tid;
     const bool live = k < N;
-    const int dbg = sa.Psm;
 
     // ---- per-CTA constants
     for (int q = tid; q < kV3NpMax; q += NT) f.BINI()[q] = q < N ? tb.bini[q] : make_int2(0, 0);
     for (int q = tid; q < kV3NpMax; q += NT) f.YY()[q] = make_double2(0.0, 0.0);
     for (int q = tid; q < kV3NpMax + 16; q += NT) f.NN()[q] = 0.0;
     for (int q = tid; q < kV3NpMax; q += NT) f.BANDV()[q] = 0.0;
+    if (vt.oDTAB) {
+        for (int q = tid; q < N; q += NT) s.DTAB[q] = tb.dtab[q];
+        for (int q = tid; q < 64; q += NT) s.EXPT[q] = tb.exptab[q];
+    }
     for (int q = tid; q < (int)(sizeof(V3Hot) / 4); q += NT)
         reinterpret_cast<uint32_t *>(smem_v3 + kV3oHOT)[q] = reinterpret_cast<const uint32_t *>(&vt.hot)[q];
     // the thread's runs (kernel parameters -> registers) and the constants of its role (v3_eval)
@@ -582,13 +559,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             sa.err[err_cell] = __longlong_as_double((long long)m);
         }
     };
-#ifdef CUDISC_PROF
-    long long *sa_prof = reinterpret_cast<long long *>(f.RED() + 96);
-    if (tid < 32) sa_prof[tid] = 0;
-    __syncthreads();
-#endif
     for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
-        PROF_T(tc0);
         const size_t row = (size_t)cell * N;
         if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, c2, k);
         prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
@@ -596,8 +567,6 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         __syncthreads();
         pc.Vg2 = s.RED[95];
         flush_err();
-        PROF_ADD(0, tc0);
-        PROF_T(tb0);
         // state and FSAL derivative of the cell (thread <-> bin) and the next cell's gas scalars: asynchronous
         // copies into (y, y m) -- free during the build -- and RED, landed by the post-build barrier
         if (live) {
@@ -630,22 +599,20 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         __syncthreads();
         tmem_fence_after();
         take_gas();
-        PROF_ADDB(11, tb0);
         // the role vectors are dead: zero the padding of the band stage (its bins are written per evaluation)
         {
-            const int padB = vt.wRow - vt.wPad - 32 * nb, npad = vt.wPad + padB, rows = 2 * vt.bandD;
+            const int padB = vt.wRow - vt.wPad - N, npad = vt.wPad + padB, rows = 2 * vt.bandD;
             for (int q = tid; q < rows * npad; q += NT) {
                 const int r = q / npad, e = q - r * npad;
-                f.WST()[r * vt.wRow + (e < vt.wPad ? e : 32 * nb + e)] = 0.0;
+                f.WST()[r * vt.wRow + (e < vt.wPad ? e : N + e)] = 0.0;
             }
         }
-        PROF_ADD(1, tb0);
 
         const bool more = cell + (int)gridDim.x < sa.C;
         if (MODE == MODE_OTF) {
             fetch_vel(cell + gridDim.x);
             const double d = v3_eval<NT>(tb, vt, f, y0, c1, c2, c3, tid, tq, more ? 4 : 0, nx, gs.mu,
-                                         gs.sigma_mol, ps, rv, colw, roww, dbg);
+                                         gs.sigma_mol, ps, rv, colw, roww);
             rv_valid = more;
             if (live) sa.out[row + k] = d;
             __syncthreads();
@@ -666,7 +633,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
                 ys = yn;
             }
             const double d = v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nx, gs.mu,
-                                         gs.sigma_mol, ps, rv, colw, roww, dbg);
+                                         gs.sigma_mol, ps, rv, colw, roww);
             if (st == 3) rv_valid = more;
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;
@@ -697,14 +664,10 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             if (lane == 0) reinterpret_cast<unsigned long long *>(s.RED)[64 + warp] = eb;
         }
         err_cell = cell;
-        PROF_ADD(8, tc0);
     }
     tmem_fence_before();
     __syncthreads();
     flush_err();
-#ifdef CUDISC_PROF
-    if (tid < 32 && sa.prof) sa.prof[48 * (size_t)blockIdx.x + tid] += sa_prof[tid];
-#endif
     if (tid < 32) tmem_dealloc_all(tbase);
 }
 

@@ -128,6 +128,7 @@ struct V3Tables {
     int nTaps, nSTaps, nExc, nExcT;
     // shared-memory byte offsets laid out by the host (the fixed ones are kV3o*)
     int oWST, oCOLP, oROWP, oK, smemBytes;
+    int oDTAB;                         // per-offset and exp tables of the pair kernel behind the row copy (0: no room, read through L1)
     int nColSlots, nRowSlots;
     uint32_t col[kV3Warps][kV3ColRuns];          // packed column runs
     uint32_t row[kV3Warps][kV3RowRuns];          // packed row runs

@@ -65,7 +65,7 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
     const int D = maxd + 1;
     t.bandD = D;
     t.wPad = (omax + 1) & ~1;
-    t.wRow = (t.wPad + Np + (-omin) + 1) & ~1;
+    t.wRow = (t.wPad + N + (-omin) + 1) & ~1;
     if (2 * D * t.wRow > 32000) { out.why = "band stage too large"; return; }
     t.nTaps = t.nSTaps = 0;
     for (auto &kv : cc) {                          // sorted by (kind, d, plane, o): fixed summation order
@@ -318,6 +318,8 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
         const int evalBytes = t.oROWP + kV3RowSlotBytes * t.nRowSlots - kV3oUNION;
         t.oK = kV3oUNION + ((std::max(kV3BuildUnionBytes, evalBytes) + 15) & ~15);
         t.smemBytes = t.oK + 16 * P;
+        t.oDTAB = 0;
+        if (t.smemBytes + 16 * N + 512 <= smem_optin) { t.oDTAB = t.smemBytes; t.smemBytes += 16 * N + 512; }   // + exp table
     }
     if (t.smemBytes > smem_optin) { out.why = "kernel of a cell does not fit shared memory"; return; }
     t.on = 1;
@@ -390,7 +392,7 @@ void v3_check(const HostTables &ht, const V3Host &v, long long bad[6])
     // layout: stage, slots and role vectors below the row copy; the band pairs are all inside the stage
     if (t.oWST != kV3oUNION || t.oCOLP < t.oWST + 8 * 2 * D * t.wRow || t.oROWP != t.oCOLP + kV3ColSlotBytes * t.nColSlots ||
         t.oROWP + kV3RowSlotBytes * t.nRowSlots > t.oK || kV3oUNION + kV3BuildUnionBytes > t.oK ||
-        t.smemBytes != t.oK + 16 * t.P) ++bad[3];
+        t.smemBytes != t.oK + 16 * t.P + (t.oDTAB ? 16 * N + 512 : 0) || (t.oDTAB && t.oDTAB != t.oK + 16 * t.P)) ++bad[3];
     for (int i = 0; i < N; ++i)
         for (int j = ht.n_bulk[i]; j <= i; ++j)
             if (i - j >= D) ++bad[4];
