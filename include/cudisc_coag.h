@@ -52,6 +52,12 @@ typedef struct {
     double sigma_mol;    /* H2 collision cross-section for nu_mol, cm^2 (reading R6; 2e-15)       */
     double rtol;         /* BS3(2) relative tolerance (default 1e-2)                */
     double atol_factor;  /* absolute tolerance = atol_factor * sum_k rho_k (1e-10)  */
+    int readings;        /* variants of two readings the paper leaves open (R2, R11); 0 = the
+                            readings taken.  Bit 0: number-conserving two-bin split (the bins
+                            receive the number fractions eps, 1 - eps of the product instead of its mass
+                            fractions).  Bit 1: the fragment l-bin is looked up with the total fragment mass
+                            m_j + min(chi m_j, m_i) instead of min(chi m_j, m_i).
+                            Other bits: CUDISC_ERR_INVALID.  Grid-only: fixed per cudisc_bins handle.     */
 } cudisc_params;
 
 /* Frozen per-cell inputs from the other solvers.  DEVICE pointers. */

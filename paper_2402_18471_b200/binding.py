@@ -28,7 +28,7 @@ class CudiscError(RuntimeError):
 class cudisc_params(C.Structure):
     _fields_ = [("mu", C.c_double), ("v_frag", C.c_double), ("alpha", C.c_double), ("eta", C.c_double),
                 ("chi_im", C.c_double), ("sigma_mol", C.c_double), ("rtol", C.c_double),
-                ("atol_factor", C.c_double)]
+                ("atol_factor", C.c_double), ("readings", C.c_int)]
 
 
 class cudisc_gas_state(C.Structure):
@@ -116,10 +116,11 @@ class Params:
     sigma_mol: float = 2.0e-15
     rtol: float = 1e-2
     atol_factor: float = 1e-10
+    readings: int = 0      # bit 0: number-conserving split, bit 1: total-mass fragment lookup (cudisc_coag.h)
 
     def c(self) -> cudisc_params:
         return cudisc_params(self.mu, self.v_frag, self.alpha, self.eta, self.chi_im, self.sigma_mol,
-                             self.rtol, self.atol_factor)
+                             self.rtol, self.atol_factor, int(self.readings))
 
 
 def _dev_ptr(t, name: str, numel: Optional[int] = None) -> int:

@@ -7,6 +7,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
+#include <cstdint>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -95,7 +96,7 @@ int make_bins(const std::vector<double> &m, const std::vector<double> &me, const
 {
     cudisc_bins b = new (std::nothrow) cudisc_bins_s();
     if (!b) return fail(CUDISC_ERR_INVALID, "out of host memory");
-    std::string why = build_tables(m, me, a, rho_m, p.eta, p.chi_im, b->ht);
+    std::string why = build_tables(m, me, a, rho_m, p.eta, p.chi_im, p.readings, b->ht);
     if (!why.empty()) { delete b; return fail(CUDISC_ERR_INVALID, "%s", why.c_str()); }
     b->magic = kBinsMagic;
     b->p = p;

@@ -20,13 +20,16 @@ struct Split {
     double eps;    // mass fraction to lo; 1 - eps to lo + 1
 };
 
-Split split_mass(const std::vector<double> &m, double mass)
+// number_split (reading R11, variant): the bins receive the NUMBER fractions eps, 1 - eps of the product,
+// i.e. the masses eps m_lo and (1 - eps) m_lo+1 (they also sum to `mass`): mass fraction eps m_lo / mass.
+Split split_mass(const std::vector<double> &m, double mass, bool number_split)
 {
     const int N = (int)m.size();
     if (mass < m[0]) return {-1, 0.0};
     if (mass >= m[N - 1]) return {N - 1, 1.0};
     int lo = (int)(std::upper_bound(m.begin(), m.end(), mass) - m.begin()) - 1;
     double eps = (m[lo + 1] - mass) / (m[lo + 1] - m[lo]);
+    if (number_split) eps = eps * m[lo] / mass;
     return {lo, eps};
 }
 
@@ -71,8 +74,14 @@ void pair_outcomes(const HostTables &t, int i, int j, bool with_columns, bool sk
         switch (coag_case(m, i, j)) {
         case COAG_NEXT: {
             double D = m[i + 1] - mi;
-            emit(i, 0, mj * (m[i + 1] - 2.0 * mi - mj) / D);
-            emit(i + 1, 0, mj * (mi + mj) / D);
+            if (t.variant & kVarNumberSplit) {
+                // number m_j / D of the product arrives in bin i + 1 (mass m_{i+1} each), the rest stays in bin i
+                emit(i, 0, -mj * mi / D);
+                emit(i + 1, 0, mj * m[i + 1] / D);
+            } else {
+                emit(i, 0, mj * (m[i + 1] - 2.0 * mi - mj) / D);
+                emit(i + 1, 0, mj * (mi + mj) / D);
+            }
             break;
         }
         case COAG_TOP:
@@ -80,7 +89,7 @@ void pair_outcomes(const HostTables &t, int i, int j, bool with_columns, bool sk
             break;
         case COAG_FAR: {
             double M = mi + mj;
-            Split s = split_mass(m, M);
+            Split s = split_mass(m, M, t.variant & kVarNumberSplit);
             emit(i, 0, -mi);
             if (s.lo == N - 1) emit(N - 1, 0, M);
             else { emit(s.lo, 0, M * s.eps); emit(s.lo + 1, 0, M * (1.0 - s.eps)); }
@@ -92,12 +101,18 @@ void pair_outcomes(const HostTables &t, int i, int j, bool with_columns, bool sk
         double m_rem = (x < mi) ? mi - x : 0.0;
         if (frag_near(m, chi, i, j)) {
             double Dp = mi - m[i - 1];
-            emit(i, 1, -x * (1.0 + m_rem / Dp));
-            emit(i - 1, 1, m_rem * x / Dp);
+            if (t.variant & kVarNumberSplit) {
+                // number chi m_j / D' of the remnant drops to bin i - 1 (mass m_{i-1} each)
+                emit(i, 1, -x * mi / Dp);
+                emit(i - 1, 1, x * m[i - 1] / Dp);
+            } else {
+                emit(i, 1, -x * (1.0 + m_rem / Dp));
+                emit(i - 1, 1, m_rem * x / Dp);
+            }
         } else {
             emit(i, 1, -mi);
             if (m_rem > 0.0) {
-                Split s = split_mass(m, m_rem);
+                Split s = split_mass(m, m_rem, t.variant & kVarNumberSplit);
                 if (s.lo == -1) emit(0, 1, m_rem);
                 else if (s.lo == N - 1) emit(N - 1, 1, m_rem);
                 else { emit(s.lo, 1, m_rem * s.eps); emit(s.lo + 1, 1, m_rem * (1.0 - s.eps)); }
@@ -114,7 +129,7 @@ void pair_outcomes(const HostTables &t, int i, int j, bool with_columns, bool sk
     if (!col_frag) {
         // largest fragment limited by the target mass: m_lf = m_i, m_ft = m_j + m_i
         if (!with_columns) emit(j, 1, -mj);        // Kf loss of bin j not in the column sum either
-        emit(N + l_bin(t.me, mi), 1, mj + mi);
+        emit(N + l_bin(t.me, (t.variant & kVarTotalLookup) ? mj + mi : mi), 1, mj + mi);
     }
 }
 
@@ -140,9 +155,10 @@ std::string build_log_grid(int N, double a_min, double a_max, double rho_m,
 }
 
 std::string build_tables(const std::vector<double> &m, const std::vector<double> &me,
-                         const std::vector<double> &a, double rho_m, double eta, double chi,
+                         const std::vector<double> &a, double rho_m, double eta, double chi, int variant,
                          HostTables &t)
 {
+    if (variant & ~(kVarNumberSplit | kVarTotalLookup)) return "unknown bits in params.readings";
     const int N = (int)m.size();
     if (N < 2) return "n_bins < 2";
     if ((int)me.size() != N + 1 || (int)a.size() != N) return "inconsistent grid arrays";
@@ -153,7 +169,7 @@ std::string build_tables(const std::vector<double> &m, const std::vector<double>
         if (!(a[k] > 0.0)) return "non-positive grain radius";
     }
     t = HostTables();
-    t.N = N; t.rho_m = rho_m; t.eta = eta; t.chi = chi;
+    t.N = N; t.rho_m = rho_m; t.eta = eta; t.chi = chi; t.variant = variant;
     t.m = m; t.me = me; t.a = a;
     t.rm.resize(N);
     for (int k = 0; k < N; ++k) t.rm[k] = 1.0 / m[k];
@@ -164,7 +180,7 @@ std::string build_tables(const std::vector<double> &m, const std::vector<double>
     for (int j = 0; j < N; ++j) {
         for (int i = j; i < N; ++i)
             if (chi * m[j] < m[i]) { t.iS[j] = i; break; }
-        t.lj[j] = l_bin(me, chi * m[j]);
+        t.lj[j] = l_bin(me, (variant & kVarTotalLookup) ? m[j] + chi * m[j] : chi * m[j]);
     }
     t.jS_lo.assign(N, 0); t.jS_hi.assign(N, 0);
     for (int l = 0; l < N; ++l) {
@@ -187,7 +203,11 @@ std::string build_tables(const std::vector<double> &m, const std::vector<double>
         t.n_bulk[i] = nb;
         if (nb == 0) continue;
         // coagulation:  Rc m_j (m_{i+1} - 2 m_i - m_j) / D -> bin i ;  Rc m_j (m_i + m_j) / D -> bin i+1
-        if (i < N - 1) {
+        if (i < N - 1 && (variant & kVarNumberSplit)) {
+            double D = m[i + 1] - m[i];             // -Rc m_j m_i / D -> bin i ;  Rc m_j m_{i+1} / D -> bin i+1
+            t.cA1[i] = -m[i] / D;
+            t.cB1[i] = m[i + 1] / D;
+        } else if (i < N - 1) {
             double D = m[i + 1] - m[i];
             t.cA1[i] = (m[i + 1] - 2.0 * m[i]) / D; t.cA2[i] = -1.0 / D;
             t.cB1[i] = m[i] / D;                    t.cB2[i] = 1.0 / D;
@@ -196,8 +216,13 @@ std::string build_tables(const std::vector<double> &m, const std::vector<double>
         }
         // fragmentation: -Rf chi m_j (1 + (m_i - chi m_j)/D') -> bin i ; Rf (m_i - chi m_j) chi m_j / D' -> i-1
         double Dp = m[i] - m[i - 1];               // nb > 0 implies i >= 1
-        t.cF1[i] = -chi * (1.0 + m[i] / Dp);  t.cF2[i] = chi * chi / Dp;
-        t.cG1[i] = chi * m[i] / Dp;           t.cG2[i] = -chi * chi / Dp;
+        if (variant & kVarNumberSplit) {           // -Rf chi m_j m_i / D' -> bin i ;  Rf chi m_j m_{i-1} / D' -> i-1
+            t.cF1[i] = -chi * m[i] / Dp;
+            t.cG1[i] = chi * m[i - 1] / Dp;
+        } else {
+            t.cF1[i] = -chi * (1.0 + m[i] / Dp);  t.cF2[i] = chi * chi / Dp;
+            t.cG1[i] = chi * m[i] / Dp;           t.cG2[i] = -chi * chi / Dp;
+        }
     }
 
     // ---- band: everything outside the bulk prefixes, plus what the column sums do not cover

@@ -28,8 +28,13 @@ struct BandEntry {
     double coef;  // contribution = coef * n_i * n_j * Kplane_ij  (diagonal K already halved)
 };
 
+// Variants of two readings the paper cannot pin (R2, R11; cudisc_params.readings)
+enum { kVarNumberSplit = 1,    // the two bins receive NUMBER fractions (masses eps m_l, (1 - eps) m_u)
+       kVarTotalLookup = 2 };  // fragment l-bin looked up with the total fragment mass
+
 struct HostTables {
     int N = 0;
+    int variant = 0;
     double rho_m = 0, eta = 0, chi = 0;
     std::vector<double> m, me, a, rm;
     // bulk row coefficients: bin i   += n_i (cA1 A1 + cA2 A2 + cF1 F1 + cF2 F2)
@@ -49,7 +54,7 @@ struct HostTables {
 std::string build_log_grid(int N, double a_min, double a_max, double rho_m,
                            std::vector<double> &m, std::vector<double> &me, std::vector<double> &a);
 std::string build_tables(const std::vector<double> &m, const std::vector<double> &me,
-                         const std::vector<double> &a, double rho_m, double eta, double chi,
+                         const std::vector<double> &a, double rho_m, double eta, double chi, int variant,
                          HostTables &out);
 
 // Expanded gather form of ALL outcomes (bulk written out pair by pair) for host-side checking;

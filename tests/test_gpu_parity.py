@@ -429,3 +429,34 @@ def test_step_host_sliced_pipeline_is_bit_identical_to_device_step():
         r, k, err_ref = orc.step_cells(*oracle_args(ds), po, r, dt, k1=k)
     assert_rho_close(a.numpy()[cells], r, 3 * TOL_RHO_1, "sliced step_host, sampled cells")
     np.testing.assert_allclose(e.numpy()[cells], err_ref, rtol=1e-6, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------ reading variants
+@pytest.mark.parametrize("readings", [1, 2, 3])
+@pytest.mark.parametrize("index,n_cells", [(1, None), (2, 24), (4, 12), (5, 6)])
+def test_reading_variants_match_oracle(index, n_cells, readings):
+    """cudisc_params.readings (number-conserving split; total-mass fragment
+    lookup) through the CUDA path -- stencil kernel (configs 1, 2, 4) and general kernel
+    (config 5) -- against the oracle with the same switch: one rate evaluation and ten steps."""
+    import dataclasses
+    cfg, d = _disc(index, n_cells)
+    po, pc = params_pair(cfg)
+    pc = dataclasses.replace(pc, readings=readings)
+    orc.set_variant(readings)
+    try:
+        g = GpuDisc(d, pc)
+        dref, _, _ = orc.rates_cells(*oracle_args(d), po, d.rho_dust)
+        gain, loss = split_free_magnitudes(d, po, cfg)
+        assert_rates_close(g.rates_otf().cpu().numpy(), dref, gain, loss, what=f"cfg{index} readings {readings}")
+        dt = dt_of(index) if index > 1 else synth_disc.YEAR
+        rho = g.rho.clone()
+        rho_ref, k_ref = d.rho_dust.copy(), None
+        for s in range(10):
+            rho_ref, k_ref, err_ref = orc.step_cells(*oracle_args(d), po, rho_ref, dt, k1=k_ref)
+            before = rho.sum(dim=1)
+            err = g.step(rho, dt)
+            assert float(((rho.sum(dim=1) - before).abs() / before).max()) <= TOL_MASS
+        assert_rho_close(rho.cpu().numpy(), rho_ref, 10 * TOL_RHO_1, f"cfg{index} readings {readings}, 10 steps")
+        np.testing.assert_allclose(err.cpu().numpy(), err_ref, rtol=1e-5, atol=1e-12)
+    finally:
+        orc.set_variant(0)

@@ -70,17 +70,28 @@ def _eval_tables(ex, N, Kc, Kf, rho, m_c):
     return d, S
 
 
+@pytest.fixture
+def oracle_variant():
+    """Sets the oracle's reading switch (R2, R11) for one test and puts it back."""
+    yield orc.set_variant
+    orc.set_variant(0)
+
+
+@pytest.mark.parametrize("readings", [0, 1, 2, 3])
 @pytest.mark.parametrize("N,a_max,chi", [(40, 1.0, 1.0), (100, 10.0, 1.0), (150, 10.0, 1.0),
                                          (24, 1e-1, 0.4), (30, 1e-2, 2.5), (12, 1e-4, 1.0), (2, 2e-5, 1.0)])
-def test_outcome_tables_reproduce_oracle_rates(N, a_max, chi):
+def test_outcome_tables_reproduce_oracle_rates(N, a_max, chi, readings, oracle_variant):
+    """readings: the library's switch for the two readings the paper leaves open (cudisc_params.readings)
+    against the oracle's own switch (orc_set_variant), both written from PAPER.md:446 and :469-476."""
     rng = np.random.default_rng(N * 7 + int(chi * 10))
-    p = cd.Params(chi_im=chi)
+    p = cd.Params(chi_im=chi, readings=readings)
     b = cd.Bins(N, 1e-5, a_max, 1.67, p)
     ex = b.expand_outcomes()
     g = orc.mass_grid(N, 1e-5, a_max, 1.67)
     K = rng.uniform(0.5, 2.0, size=(N, N)); K = 0.5 * (K + K.T)
     pf = rng.uniform(0.0, 1.0, size=(N, N)); pf = 0.5 * (pf + pf.T)
     rho = 10.0 ** rng.uniform(-3, 0, size=N)
+    oracle_variant(readings)
     d_ref, gain, loss, S_ref = orc.rates_flux(g, K, pf, rho, chi=chi)
     d, S = _eval_tables(ex, N, K * (1 - pf), K * pf, rho, g.m_c)
     np.testing.assert_allclose(S, S_ref, rtol=1e-12, atol=1e-300)
@@ -102,6 +113,22 @@ def test_general_grid_tables_match_log_grid_tables():
     for k in e1:
         np.testing.assert_array_equal(e1[k], e2[k])
     np.testing.assert_allclose(b2.query()["a_centres"], q["a_centres"], rtol=1e-14)
+
+
+def test_readings_bits_are_validated():
+    with pytest.raises(cd.CudiscError):
+        cd.Bins(40, 1e-5, 1.0, 1.67, cd.Params(readings=4))
+
+
+@pytest.mark.parametrize("readings", [1, 2, 3])
+def test_stencil_kernel_takes_the_reading_variants(readings):
+    """The run lists and the band stencil of the cell kernel are rebuilt from the variant's tables and
+    re-checked against them (coag_v3.h v3_check)."""
+    b = cd.Bins(150, 1e-5, 10.0, 1.67, cd.Params(readings=readings))
+    out = b.schedule_check()
+    assert out[:6] == [0, 0, 0, 0, 0, 0], out
+    on, smem, tmem = b.fast_path()
+    assert on and smem <= 227 * 1024
 
 
 @pytest.mark.parametrize("n_bins,a_min,a_max", [(2, 1e-5, 1.0), (3, 1e-5, 1e-3), (31, 1e-5, 1.0), (32, 1e-5, 1.0),
