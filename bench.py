@@ -308,11 +308,14 @@ def run_ours(args):
                     "api": "cudisc_coag_step_host (pinned host buffers)"},
             "gpu_launches": int(launches),
             "roofline": {
-                "bound": "alu", "kernel": "cudisc::coag_cells_kernel<512, MODE_STEP, false>",
+                "bound": "alu",
+                "kernel": "cudisc::coag_v3_kernel<512, MODE_STEP>" if bins.fast_path()[0] else
+                          "cudisc::coag_cells_kernel<512, MODE_STEP, SLAB, false>",
                 "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops,
-                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, profiles/r01_v7_step_kernel.md
-                "traffic": 193176832 if (args.config == 4 and world == 1) else None,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch (ncu --set full), profiles/r02_kernels.md
+                "traffic": 194343680 if (args.config == 4 and world == 1) else
+                           (1226387200 if (args.config == 5 and world == 1) else None),
                 "how": f"algorithmic FP64 instructions per launch = C*P*({I_BUILD} + {EVALS_PER_STEP}*{I_EVAL}) "
                        f"= {alg_instr:.4g} (DESIGN.md 'Roofline'), x2 flop per FP64 issue slot, / mean CUDA-event "
                        f"launch duration {1e3 * kernel_s:.3f} ms; peak = {sm_count} SMs x {FP64_LANES_PER_SM} "
@@ -321,9 +324,10 @@ def run_ours(args):
                 "frac_of_measured_dfma": achieved_tflops / (2.0 * dfma_per_s / 1e12),
                 "hbm_copy_measured_gbs": copy_bps / 1e9,
                 "hbm_algorithmic_gbs": (6.0 * C * N * 8 + 5.0 * C * 8) / kernel_s / 1e9,
-                "note": "the FP64 pipe is the roofline BASELINE.json names; ncu (profiles/) shows the kernel is "
-                        "limited by the shared-memory data pipe (K store read twice per rate evaluation), "
-                        "see DESIGN.md 'Roofline'",
+                "note": "the FP64 pipe is the roofline BASELINE.json names; frac is the share of FP64 issue slots the "
+                        "algorithmic instructions would need, not a FLOP/s claim.  ncu (profiles/r02_kernels.md): the "
+                        "kernel is latency-bound (16 warps per SM, issue slots 48 %, FP64 pipe 28 %, shared-memory pipe "
+                        "49 %), see DESIGN.md 'Roofline'",
             },
         }
         if world == 1 and not args.no_cpu_baseline:
