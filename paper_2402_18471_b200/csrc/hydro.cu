@@ -2,14 +2,16 @@
 // Eqs. 32-37) for sm_100a: cudisc_hydro_create / cudisc_hydrostatic / cudisc_hydro_destroy.
 //
 // This is the step that produces the rho_gas the coagulation path consumes.  It is
-// HBM-bound: 8 B read (c_s^2) and 8 B written (rho_g) per cell.  One warp owns one radial column at a
-// time (columns are contiguous in memory: j, the Z index, runs fastest):
+// HBM-bound: 8 B read (c_s^2) and 8 B written (rho_g) per cell.  One CTA owns one radial column at a
+// time (columns are contiguous in memory: j, the Z index, runs fastest), four consecutive cells per thread:
 //   * the column of c_s^2 arrives in shared memory by a 1-D bulk copy (cp.async.bulk, the TMA engine)
-//     completing on an mbarrier; the copy of the warp's NEXT column is in flight while it works;
-//   * per 32 cells: the pressure ratios of Eq. 34 (IEEE sqrt / divide in the paper's operation order,
-//     exp), a multiplicative inclusive scan over the lanes in a fixed order (Eq. 36) times the carry of
-//     the previous 32, omega = P / c_s^2, the lane's share of sum_k omega V (Eq. 37);
+//     completing on an mbarrier; the copy of the CTA's NEXT column is in flight while it works;
+//   * per cell the pressure ratio of Eq. 34 (IEEE divide in the paper's operation order, exp); Eq. 36 as a
+//     product inside the thread, a multiplicative scan over the lanes and one over the warps, all in a fixed
+//     order; omega = P / c_s^2; sum_k omega V by a block reduction (Eq. 37);
 //   * the normalised densities leave through a bulk store from shared memory.
+// (Round 1 of this kernel gave a whole column to one warp: 14 warps per SM, one latency chain per 128 cells,
+//  0.13 of the HBM rate.)
 // Written from the paper; shares nothing with oracle/.
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -65,111 +67,126 @@ __device__ __forceinline__ void bulk_store(void *dst_gmem, const void *src_smem,
 __device__ __forceinline__ void bulk_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 
-// TMA = true: n_z even (16-byte columns): bulk copies through shared memory; else plain loads / stores.
-// Four groups of 32 cells are in flight per warp (their ratios and lane scans are independent; only the
-// carry of Eq. 36 chains them), which is what hides the divide / exp / shuffle latencies.
+// One CTA per radial column at a time, 4 consecutive cells per thread (blockDim = ceil(n_z / 4) rounded up to a
+// warp, <= 1024).  TMA = true (n_z even, 16-byte aligned arrays): the column of c_s^2 arrives in shared memory by a
+// 1-D bulk copy completing on an mbarrier, the CTA's NEXT column in flight meanwhile, and the densities leave
+// through a bulk store; else plain loads / stores.  The product of Eq. 36 is taken in a fixed order: within the
+// thread, then a multiplicative scan over the lanes, then over the warps.
+constexpr int kHU = 4;
+
 template <bool TMA>
-__global__ void __launch_bounds__(512) hydro_kernel(const HydroGeom gm, const double *__restrict__ cs2,
-                                                    const double *__restrict__ Sigma, double GM,
-                                                    double *__restrict__ rho)
+__global__ void __launch_bounds__(1024) hydro_kernel(const HydroGeom gm, const double *__restrict__ cs2,
+                                                     const double *__restrict__ Sigma, double GM,
+                                                     double *__restrict__ rho)
 {
     extern __shared__ __align__(16) double hs[];
-    constexpr int U = 4;
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
     const int n_z = gm.n_z, nzp = (n_z + 1) & ~1;
-    // per warp: two column buffers (the densities overwrite the sound speeds in place), 2 mbarriers
-    double *in0 = hs + (size_t)wib * (2 * nzp + 2), *in1 = in0 + nzp;
-    uint64_t *bar = reinterpret_cast<uint64_t *>(in1 + nzp);
-    const int gw = blockIdx.x * wpb + wib, nw = gridDim.x * wpb;
+    double *buf0 = hs, *buf1 = hs + nzp;
+    double *edge = hs + 2 * nzp;                 // [2][32] last 1/r, 1/c_s^2 of every warp
+    double *wtot = edge + 64;                    // [32] warp products
+    double *wsum = wtot + 32;                    // [32] warp sums of omega V
+    uint64_t *bar = reinterpret_cast<uint64_t *>(wsum + 32);
     const uint32_t bytes = (uint32_t)n_z * 8u;
-    if (TMA) {
-        if (lane == 0) { mbar_init(bar, 1); mbar_init(bar + 1, 1); }
-        __syncwarp();
+    if (TMA && tid == 0) {
+        mbar_init(bar, 1); mbar_init(bar + 1, 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-        if (lane == 0 && gw < gm.n_r) { mbar_expect_tx(bar, bytes); bulk_load(in0, cs2 + (size_t)gw * n_z, bytes, bar); }
+        if ((int)blockIdx.x < gm.n_r) { mbar_expect_tx(bar, bytes); bulk_load(buf0, cs2 + (size_t)blockIdx.x * n_z, bytes, bar); }
     }
+    __syncthreads();
     uint32_t ph0 = 0u, ph1 = 0u;
-    int buf = 0;
-    for (int i = gw; i < gm.n_r; i += nw, buf ^= 1) {
-        double *c;                                       // column buffer: c_s^2 in, rho out
+    int b = 0;
+    const int j0 = kHU * tid;
+    for (int i = blockIdx.x; i < gm.n_r; i += gridDim.x, b ^= 1) {
+        double *c = b ? buf1 : buf0;             // column buffer: c_s^2 in, rho out
         if (TMA) {
-            const int inext = i + nw;
-            bulk_store_wait_read();                      // the previous column's store has read the other buffer
-            if (lane == 0 && inext < gm.n_r) {
-                fence_async_smem();
-                mbar_expect_tx(bar + (buf ^ 1), bytes);
-                bulk_load(buf ? in0 : in1, cs2 + (size_t)inext * n_z, bytes, bar + (buf ^ 1));
+            const int inext = i + gridDim.x;
+            if (tid == 0) {
+                bulk_store_wait_read();          // the previous column's store has read the other buffer
+                if (inext < gm.n_r) {
+                    fence_async_smem();
+                    mbar_expect_tx(bar + (b ^ 1), bytes);
+                    bulk_load(b ? buf0 : buf1, cs2 + (size_t)inext * n_z, bytes, bar + (b ^ 1));
+                }
             }
-            mbar_wait(bar + buf, buf ? ph1 : ph0);
-            if (buf) ph1 ^= 1u; else ph0 ^= 1u;
-            c = buf ? in1 : in0;
-            __syncwarp();
-        } else {
-            c = rho + (size_t)i * n_z;                   // results are staged in the output column
+            mbar_wait(bar + b, b ? ph1 : ph0);
+            if (b) ph1 ^= 1u; else ph0 ^= 1u;
         }
         const double *cin = TMA ? c : cs2 + (size_t)i * n_z;
         const double Rc = gm.Rc[i], dR3 = gm.dR3[i];
-        double carry = 1.0, part = 0.0, inv_r_last = 0.0, inv_c_last = 0.0;
-        for (int j0 = 0; j0 < n_z; j0 += 32 * U) {
-            double cj[U], inv_r[U], inv_c[U], p[U];
-            bool act[U];
+        double cj[kHU], inv_r[kHU], inv_c[kHU], p[kHU];
+        bool act[kHU];
 #pragma unroll
-            for (int u = 0; u < U; ++u) {
-                const int j = j0 + 32 * u + lane;
-                act[u] = j < n_z;
-                cj[u] = act[u] ? cin[j] : 1.0;
-                const double r = __dmul_rn(Rc, act[u] ? gm.sj[j] : 1.0);
-                inv_r[u] = __ddiv_rn(1.0, r);
-                inv_c[u] = __ddiv_rn(1.0, cj[u]);
+        for (int u = 0; u < kHU; ++u) {
+            const int j = j0 + u;
+            act[u] = j < n_z;
+            cj[u] = act[u] ? cin[j] : 1.0;
+            const double r = __dmul_rn(Rc, act[u] ? gm.sj[j] : 1.0);
+            inv_r[u] = __drcp_rn(r);             // == 1.0 / r, correctly rounded
+            inv_c[u] = __drcp_rn(cj[u]);
+        }
+        // the previous cell's 1/r, 1/c_s^2 of the thread's first cell: the neighbour lane, or the last lane of
+        // the previous warp through shared memory
+        double pr = __shfl_up_sync(0xffffffffu, inv_r[kHU - 1], 1), pc = __shfl_up_sync(0xffffffffu, inv_c[kHU - 1], 1);
+        if (lane == 31) { edge[warp] = inv_r[kHU - 1]; edge[32 + warp] = inv_c[kHU - 1]; }
+        __syncthreads();
+        if (lane == 0 && warp > 0) { pr = edge[warp - 1]; pc = edge[32 + warp - 1]; }
+        double q = 1.0;                          // running product inside the thread
+#pragma unroll
+        for (int u = 0; u < kHU; ++u) {
+            const double r_prev = u ? inv_r[u - 1] : pr, c_prev = u ? inv_c[u - 1] : pc;
+            double ratio = 1.0;
+            if (act[u] && j0 + u > 0) {
+                const double avg = __dmul_rn(0.5, __dadd_rn(inv_c[u], c_prev));                    // Eq. 35
+                ratio = exp(__dmul_rn(__dmul_rn(GM, avg), __dsub_rn(inv_r[u], r_prev)));         // Eq. 34
             }
+            q *= ratio;
+            p[u] = q;
+        }
+        // Eq. 36: exclusive multiplicative scan of the thread products over the lanes, then over the warps
+        double incl = q;
 #pragma unroll
-            for (int u = 0; u < U; ++u) {
-                double inv_r_prev = __shfl_up_sync(0xffffffffu, inv_r[u], 1);
-                double inv_c_prev = __shfl_up_sync(0xffffffffu, inv_c[u], 1);
-                const double rl = u ? __shfl_sync(0xffffffffu, inv_r[u ? u - 1 : 0], 31) : inv_r_last;
-                const double cl = u ? __shfl_sync(0xffffffffu, inv_c[u ? u - 1 : 0], 31) : inv_c_last;
-                if (lane == 0) { inv_r_prev = rl; inv_c_prev = cl; }
-                p[u] = 1.0;
-                if (act[u] && j0 + 32 * u + lane > 0) {
-                    const double avg = __dmul_rn(0.5, __dadd_rn(inv_c[u], inv_c_prev));                // Eq. 35
-                    p[u] = exp(__dmul_rn(__dmul_rn(GM, avg), __dsub_rn(inv_r[u], inv_r_prev)));     // Eq. 34
-                }
+        for (int o = 1; o < 32; o <<= 1) {
+            const double v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl *= v;
+        }
+        double excl = __shfl_up_sync(0xffffffffu, incl, 1);
+        if (lane == 0) excl = 1.0;
+        if (lane == 31) wtot[warp] = incl;
+        __syncthreads();
+        double carry = 1.0;
+        for (int w = 0; w < warp; ++w) carry *= wtot[w];
+        carry *= excl;
+        double part = 0.0;
+#pragma unroll
+        for (int u = 0; u < kHU; ++u) {
+            if (act[u]) {
+                const int j = j0 + u;
+                const double omega = __dmul_rn(__dmul_rn(p[u], carry), inv_c[u]);     // P / c_s^2 (one extra rounding)
+                part = fma(omega, dR3 * gm.dtan3[j], part);                                        // Eq. 1
+                p[u] = omega;
             }
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {                                                       // Eq. 36
-#pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    const double v = __shfl_up_sync(0xffffffffu, p[u], o);
-                    if (lane >= o) p[u] *= v;
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                p[u] *= carry;
-                carry = __shfl_sync(0xffffffffu, p[u], 31);
-                if (act[u]) {
-                    const int j = j0 + 32 * u + lane;
-                    const double omega = __ddiv_rn(p[u], cj[u]);
-                    const double V = dR3 * gm.dtan3[j];                                              // Eq. 1
-                    part = fma(omega, V, part);
-                    c[j] = omega;
-                }
-            }
-            inv_r_last = __shfl_sync(0xffffffffu, inv_r[U - 1], 31);
-            inv_c_last = __shfl_sync(0xffffffffu, inv_c[U - 1], 31);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-        const double norm = __ddiv_rn(__dmul_rn(Sigma[i], gm.RdR[i]), part);                         // Eq. 37
-        __syncwarp();
-        for (int j = lane; j < n_z; j += 32) c[j] = __dmul_rn(c[j], norm);
+        if (lane == 0) wsum[warp] = part;
+        __syncthreads();
+        double tot = 0.0;
+        for (int w = 0; w < nwarps; ++w) tot += wsum[w];
+        const double norm = __ddiv_rn(__dmul_rn(Sigma[i], gm.RdR[i]), tot);                        // Eq. 37
+        double *o = TMA ? c : rho + (size_t)i * n_z;
+#pragma unroll
+        for (int u = 0; u < kHU; ++u)
+            if (act[u]) o[j0 + u] = __dmul_rn(p[u], norm);
         if (TMA) {
             fence_async_smem();
-            __syncwarp();
-            if (lane == 0) bulk_store(rho + (size_t)i * n_z, c, bytes);
+            __syncthreads();
+            if (tid == 0) bulk_store(rho + (size_t)i * n_z, c, bytes);
+        } else {
+            __syncthreads();                     // edge / wtot / wsum are free for the next column
         }
     }
-    if (TMA) bulk_store_wait_read();
+    if (TMA && tid == 0) bulk_store_wait_read();
 }
 
 thread_local char h_err[256] = "";
@@ -259,25 +276,26 @@ int cudisc_hydrostatic(cudisc_hydro h, const double *cs2, const double *Sigma_g,
     if (cs2 == rho_gas_out) return hfail(CUDISC_ERR_INVALID, "cs2 and rho_gas_out may not alias");
     const int n_z = h->n_z, nzp = (n_z + 1) & ~1;
     const bool tma = (n_z % 2 == 0) && ((uintptr_t)cs2 % 16 == 0) && ((uintptr_t)rho_gas_out % 16 == 0);
-    const size_t per_warp = (size_t)(2 * nzp + 2) * sizeof(double);
-    int wpb = 16;
-    while (wpb > 1 && wpb * per_warp > (size_t)h->smem_optin - 1024) --wpb;
-    const size_t smem = tma ? wpb * per_warp : 0;
-    const int blocks = std::max(1, std::min((h->n_r + wpb - 1) / wpb, 8 * h->sms));
+    const int threads = std::min(1024, ((n_z + kHU - 1) / kHU + 31) & ~31);
+    const size_t smem = (size_t)(2 * nzp + 64 + 32 + 32 + 2) * sizeof(double);
+    // resident CTAs per SM: threads and shared memory (registers: 64 per thread)
+    const int per_sm = std::max(1, std::min({2048 / threads, (int)((size_t)h->smem_optin / (smem + 1024)), 65536 / (64 * threads)}));
+    const int blocks = std::max(1, std::min(h->n_r, per_sm * h->sms));
     cudaError_t e = cudaSuccess;
-    if (tma) {
+    {
         static bool attr_done[64] = {false};
         int dev = 0;
         e = cudaGetDevice(&dev);
         if (e == cudaSuccess && (dev < 0 || dev >= 64 || !attr_done[dev])) {
             e = cudaFuncSetAttribute(hydro_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin);
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(hydro_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin);
             if (e == cudaSuccess && dev >= 0 && dev < 64) attr_done[dev] = true;
         }
         if (e != cudaSuccess) return hfail(CUDISC_ERR_CUDA, "hydro attribute: %s", cudaGetErrorString(e));
-        hydro_kernel<true><<<blocks, 32 * wpb, smem, (cudaStream_t)stream>>>(h->gm, cs2, Sigma_g, GM, rho_gas_out);
-    } else {
-        hydro_kernel<false><<<blocks, 32 * wpb, 0, (cudaStream_t)stream>>>(h->gm, cs2, Sigma_g, GM, rho_gas_out);
     }
+    if (tma) hydro_kernel<true><<<blocks, threads, smem, (cudaStream_t)stream>>>(h->gm, cs2, Sigma_g, GM, rho_gas_out);
+    else hydro_kernel<false><<<blocks, threads, smem, (cudaStream_t)stream>>>(h->gm, cs2, Sigma_g, GM, rho_gas_out);
     e = cudaGetLastError();
     if (e != cudaSuccess) return hfail(CUDISC_ERR_CUDA, "hydro launch: %s", cudaGetErrorString(e));
     cudisc_count_launch_();
