@@ -85,6 +85,8 @@ typedef struct {
  * of Eqs. 63-65, remnant / fragment masses of Eq. 68, l-bins and N_k of Eq. 67) from p.eta and
  * p.chi_im, on the host; they are uploaded to the current CUDA device on first use.
  * p is stored: cudisc_coag_step uses it.  Works without a CUDA device (tables stay on the host).
+ * One device per handle: the device copy of the tables follows the CURRENT device of the call that needs it,
+ * so a bins handle (and the grids made from it) must be used from one device only; use one handle per device.
  * Errors: INVALID (n_bins < 2, a_min <= 0, a_min >= a_max, rho_m <= 0, eta >= 2, chi_im <= 0,
  * out == NULL), UNSUPPORTED (n_bins > 256). */
 int cudisc_bins_create(int n_bins, double a_min, double a_max, double rho_m,

@@ -233,10 +233,12 @@ def _run_manual(N, C, seed, n_r=None, n_z=None, m_centres=None, m_edges=None, st
         assert abs(y[c].sum() - m0) <= steps * TOL_MASS * m0
 
 
-@pytest.mark.parametrize("N,C", [(2, 3), (33, 5), (64, 200), (256, 4)])
+@pytest.mark.parametrize("N,C", [(2, 3), (33, 5), (40, 7), (64, 200), (135, 160), (152, 9), (153, 5), (256, 4)])
 def test_edge_sizes_log_grid(N, C):
-    """Minimum bin count, a ragged 32-multiple, more cells than SMs, and the maximum bin count
-    (band tables too long for tensor memory -> global-table gather; K store partly in the L2 slab)."""
+    """Minimum bin count, a ragged 32-multiple, the smallest and the largest grid of the stencil kernel (40 and 152
+    bins: at 153 the cell no longer fits shared memory and the general kernel takes over), the paper's 135-bin
+    grid on more cells than SMs, and the maximum bin count (band tables too long for tensor memory -> global-table
+    gather; K store partly in the L2 slab)."""
     _run_manual(N, C, seed=100 + N, steps=2)
 
 
