@@ -346,10 +346,16 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
     }
     __syncthreads();
 
-    // ---- phase A: the bin-owning warps stage the band products of their bins and run a third of the NEXT
-    //      cell's prologue (ppart 1, 2, 3; 4: all of it); then every warp its own runs
+    // ---- phase A: the bin-owning warps stage the band products of their bins (and sum the stencil exceptions of
+    //      their bins when those only read the warp's own stage entries), run a third of the NEXT cell's prologue
+    //      (ppart 1, 2, 3; 4: all of it); then every warp its own runs
+    double excA = 0.0;          // density exceptions of the thread's own bin, summed in phase A when they are local
     if (warp < nb) {
         v3_stage(vt, f, k, live ? y : 0.0);
+        if (vt.excLocal) {
+            __syncwarp();
+            excA = v3_exceptions(f, f.WST(), warp, 0, lane, 0.0);
+        }
         if (ppart) {
             if (ppart == 1 || ppart == 4) ps = prologue_begin(tb, nx, mu, sigma_mol, k);
             prologue_newton(ps, ppart == 4 ? 6 : 2);
@@ -394,7 +400,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         if (lane == 31) eUp[warp] = dp1;
         up = __shfl_up_sync(0xffffffffu, dp1, 1);
         dn = __shfl_down_sync(0xffffffffu, dm1, 1);
-        bandR = v3_taps(f, wst, min(k, N - 1), 0, vt.nTaps >> 1);
+        bandR = v3_taps(f, wst, min(k, N - 1), 0, vt.nTapsR);
     } else if (warp < 2 * nb) {
         const int g = warp - nb, kc = 32 * g + lane;
         const double2 *colp = reinterpret_cast<const double2 *>(f.base + vt.oCOLP);
@@ -413,7 +419,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
 #pragma unroll 1
             for (int q = 0; q < vt.nSTaps; ++q) sl = fma(f.HOT()->staps[q].c, wst[f.HOT()->staps[q].off + min(kc, N - 1)], sl);
         }
-        sl = v3_exceptions(f, wst, g, 1, lane, sl);
+        if (vt.nExcS) sl = v3_exceptions(f, wst, g, 1, lane, sl);
         if (kc < N) {
             const int2 bi = f.BINI()[kc];
             double gc, h;
@@ -436,8 +442,8 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         if (kc < N) f.YY()[kc].y = suf;
     } else if (warp < 3 * nb) {
         const int g = warp - 2 * nb, t = 32 * g + lane;
-        double da = v3_taps(f, wst, min(t, N - 1), vt.nTaps >> 1, vt.nTaps);       // (the list is padded to a multiple of 8)
-        da = v3_exceptions(f, wst, g, 0, lane, da);
+        double da = v3_taps(f, wst, min(t, N - 1), vt.nTapsR, vt.nTaps);       // (the list is padded to a multiple of 8)
+        if (!vt.excLocal) da = v3_exceptions(f, wst, g, 0, lane, da);
         f.BANDV()[t] = da;
     }
     __syncthreads();
@@ -452,7 +458,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         d = d0;
         if (k > 0) d += prev;
         if (k < N - 1) d += next;
-        d += bandR + f.BANDV()[k];
+        d += (bandR + excA) + f.BANDV()[k];
         d = fma(-y, f.NN()[k], d);
         d = fma(c3, suf, d);
     }

@@ -15,8 +15,8 @@
 //
 // Band as a stencil.  coag_tables.cpp lists every outcome that the bulk row / column sums do not cover as
 // gather entries (target, i, j, plane, coef).  On a grid with constant mass ratio coef / m_i depends only on
-// (d = i - j, o = target - i, plane, kind) away from the grid ends.  Per evaluation the bin-owning threads
-// stage   W[plane][d][i] = y_i n_{i-d} Kplane[i][i-d]   (y_i = m_i n_i; d < bandD) in shared memory, and
+// (d = i - j, o = target - i, plane, kind) away from the grid ends.  Per evaluation one warp group
+// stages  W[plane][d][i] = y_i n_{i-d} Kplane[i][i-d]   (y_i = m_i n_i; d < bandD) in shared memory, and
 //   dens[t] = sum_taps c W[plane][d][t - o],   S[t] likewise,
 // with warp-uniform coefficients from the constant bank, plus a short list of exception entries at the grid
 // ends that carries the residual coefficients.  The host re-expands taps + exceptions and checks them against
@@ -126,6 +126,10 @@ struct V3Tables {
     int wRow;                          // entries per (plane, d) row of the W stage; entry of bin i at wPad + i
     int wPad;
     int nTaps, nSTaps, nExc, nExcT;
+    int nTapsR;                        // taps [0, nTapsR) go to combine group R, the rest to group D (multiples of 4)
+    int nExcS;                         // exception entries of S targets (kind 1)
+    int excLocal;                      // 1: every density exception reads stage entries of its target's own 32-bin block, so
+                                       //    the warp that staged the block sums them right away (phase A)
     // shared-memory byte offsets laid out by the host (the fixed ones are kV3o*)
     int oWST, oCOLP, oROWP, oK, smemBytes;
     int oDTAB;                         // per-offset and exp tables of the pair kernel behind the row copy (0: no room, read through L1)

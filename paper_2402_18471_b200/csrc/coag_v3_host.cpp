@@ -17,8 +17,8 @@ namespace {
 constexpr double kCBuildRow = 95.0, kCBuildFold = 120.0, kCBuildDiagCopy = 320.0;
 constexpr double kCColChunk = 450.0, kCColRun = 150.0;
 constexpr double kCRowRect = 70.0, kCRowRag = 110.0, kCRowRun = 300.0;
-constexpr double kCStage = 500.0;          // band stage of the warp's own bins
-constexpr double kCProlPiece = 1700.0;     // a third of the next cell's prologue, on the bin-owning warps
+constexpr double kCStage = 500.0;          // band stage of 32 bins (warps of combine group D)
+constexpr double kCProlPiece = 2900.0;     // a third of the next cell's prologue, on the bin-owning warps
 
 struct Key {
     int kind, d, plane, o;
@@ -117,6 +117,14 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
         if (t.nTaps >= kV3MaxTaps) { out.why = "too many stencil taps"; return; }
         V3Tap z; z.c = 0.0; z.off = t.wPad; z.pad = 0;
         t.hot.taps[t.nTaps++] = z;
+    }
+    t.nTapsR = (2 * t.nTaps / 5) & ~3;
+    t.nExcS = 0; t.excLocal = 1;
+    for (int q = 0; q < t.nExc; ++q) {
+        const V3Exc &x = t.hot.exc[q];
+        if (x.kind == 1) { t.nExcS++; continue; }
+        const int i = (x.off % t.wRow) - t.wPad;
+        if ((i >> 5) != (x.t >> 5)) t.excLocal = 0;
     }
     // exception entries by target: one warp sums the (at most 32) entries of a target with a fixed shuffle tree
     t.nExcT = 0;
