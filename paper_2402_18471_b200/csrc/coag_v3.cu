@@ -330,7 +330,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
                                           double c1, double c2, double c3, int tid, uint32_t tq, int ppart,
                                           const CellGas &nx, double mu, double sigma_mol, ProlState &ps,
                                           RoleVals &rv, const uint32_t (&colw)[kV3ColRuns],
-                                          const uint32_t (&roww)[kV3RowRuns])
+                                          const uint32_t (&roww)[kV3RowRuns], bool storeNext, double nvR, double nvZ)
 {
     const int N = vt.N, nb = vt.nb;
     const int lane = tid & 31, warp = tid >> 5;
@@ -447,6 +447,15 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         f.BANDV()[t] = da;
     }
     __syncthreads();
+    // last evaluation of a cell: the partial sums are consumed, so the role vectors of the NEXT cell go into the
+    // union now and the other warps start its build while the bin owners assemble and finish this cell
+    if (storeNext) {
+        if (warp < nb) {
+            prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, f.s, k);
+            if (tid == 0) f.RED()[95] = rv.Vg2;
+        }
+        __syncthreads();
+    }
     if (warp >= nb) return 0.0;
 
     double d = 0.0;
@@ -567,12 +576,13 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     };
     for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
         const size_t row = (size_t)cell * N;
-        if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, c2, k);
-        prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
-        if (tid == 0) s.RED[95] = rv.Vg2;
-        __syncthreads();
+        if (!rv_valid) {                              // first cell of the CTA: nothing ran ahead
+            rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, c2, k);
+            prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
+            if (tid == 0) s.RED[95] = rv.Vg2;
+            __syncthreads();
+        }
         pc.Vg2 = s.RED[95];
-        flush_err();
         // state and FSAL derivative of the cell (thread <-> bin) and the next cell's gas scalars: asynchronous
         // copies into (y, y m) -- free during the build -- and RED, landed by the post-build barrier
         if (live) {
@@ -605,6 +615,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         __syncthreads();
         tmem_fence_after();
         take_gas();
+        flush_err();
         // the role vectors are dead: zero the padding of the band stage (its bins are written per evaluation)
         {
             const int padB = vt.wRow - vt.wPad - N, npad = vt.wPad + padB, rows = 2 * vt.bandD;
@@ -618,10 +629,9 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         if (MODE == MODE_OTF) {
             fetch_vel(cell + gridDim.x);
             const double d = v3_eval<NT>(tb, vt, f, y0, c1, c2, c3, tid, tq, more ? 4 : 0, nx, gs.mu,
-                                         gs.sigma_mol, ps, rv, colw, roww);
+                                         gs.sigma_mol, ps, rv, colw, roww, more, nvR, nvZ);
             rv_valid = more;
             if (live) sa.out[row + k] = d;
-            __syncthreads();
             continue;
         }
 
@@ -639,7 +649,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
                 ys = yn;
             }
             const double d = v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nx, gs.mu,
-                                         gs.sigma_mol, ps, rv, colw, roww);
+                                         gs.sigma_mol, ps, rv, colw, roww, more && st == 3, nvR, nvZ);
             if (st == 3) rv_valid = more;
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;

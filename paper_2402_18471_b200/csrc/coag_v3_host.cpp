@@ -14,7 +14,7 @@ namespace cudisc {
 namespace {
 
 // cost model (cycles of one warp; measured ratios on B200, only the ratios matter)
-constexpr double kCBuildRow = 95.0, kCBuildFold = 120.0, kCBuildDiagCopy = 320.0;
+constexpr double kCBuildRow = 95.0, kCBuildFold = 120.0, kCBuildDiagCopy = 320.0, kCBuildOwnerLate = 250.0;
 constexpr double kCColChunk = 450.0, kCColRun = 150.0;
 constexpr double kCRowRect = 70.0, kCRowRag = 110.0, kCRowRun = 300.0;
 constexpr double kCStage = 500.0;          // band stage of 32 bins (warps of combine group D)
@@ -174,11 +174,14 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
             total += kCBuildRow * rows;
         }
     }
+    total += kCBuildOwnerLate * nb;
     const double T = total / kV3Warps;
     std::vector<std::vector<Chunk>> mine(kV3Warps);
     double load[kV3Warps] = {0};
     int qfill[4] = {0, 0, 0, 0};
     int diagWarp[kV3MaxBlk];
+    // the bin-owning warps join the build late: they assemble and finish the previous cell first (coag_v3.cu)
+    for (int w = 0; w < nb; ++w) load[w] = kCBuildOwnerLate;
     for (int c = 0; c < nb; ++c) {
         const int w = kV3Warps - 1 - c;                 // away from the bin-owning warps
         diagWarp[c] = w;
