@@ -17,6 +17,15 @@
 // One persistent CTA of 512 threads per SM; thread k < N owns bin k (state and derivatives in registers).
 #include "coag_v3.h"
 #include "coag_launch.h"
+#ifndef V3X_R
+#define V3X_R 1
+#endif
+#ifndef V3X_C
+#define V3X_C 1
+#endif
+#ifndef V3X_D
+#define V3X_D 1
+#endif
 
 namespace cudisc {
 
@@ -304,22 +313,38 @@ __device__ __forceinline__ double v3_exceptions(const VSm &f, const double *wst,
     return acc;
 }
 
-// band stencil of target t over taps [q0, q1) (multiples of 4): 4 loads in flight per batch
+// band stencil of target t over density taps [q0, q1) (multiples of 8) / over the S taps.  A tap is one 16-byte
+// load from the table in shared memory; the eight stage loads of a batch are in flight together.
 __device__ __forceinline__ double v3_taps(const VSm &f, const double *wst, int t, int q0, int q1)
 {
-    const V3Hot *hot = f.HOT();
-    double da = 0.0, db = 0.0;
+    const double *w = wst + t;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
 #pragma unroll 1
-    for (int q = q0; q < q1; q += 4) {
-        double w4[4];
+    for (int q = q0; q < q1; q += 8) {
+        const uint4 *tp = reinterpret_cast<const uint4 *>(f.HOT()->taps + q);
+        uint4 e[8];
+        double v[8];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) w4[u] = wst[hot->taps[q + u].off + t];
-        da = fma(hot->taps[q].c, w4[0], da);
-        db = fma(hot->taps[q + 1].c, w4[1], db);
-        da = fma(hot->taps[q + 2].c, w4[2], da);
-        db = fma(hot->taps[q + 3].c, w4[3], db);
+        for (int u = 0; u < 8; ++u) e[u] = tp[u];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = w[(int)e[u].z];
+        a0 = fma(u2d(e[0].x, e[0].y), v[0], a0); a1 = fma(u2d(e[1].x, e[1].y), v[1], a1);
+        a2 = fma(u2d(e[2].x, e[2].y), v[2], a2); a3 = fma(u2d(e[3].x, e[3].y), v[3], a3);
+        a0 = fma(u2d(e[4].x, e[4].y), v[4], a0); a1 = fma(u2d(e[5].x, e[5].y), v[5], a1);
+        a2 = fma(u2d(e[6].x, e[6].y), v[6], a2); a3 = fma(u2d(e[7].x, e[7].y), v[7], a3);
     }
-    return da + db;
+    return (a0 + a1) + (a2 + a3);
+}
+__device__ __forceinline__ double v3_staps(const V3Tables &vt, const VSm &f, const double *wst, int t)
+{
+    const double *w = wst + t;
+    double a0 = 0.0;
+#pragma unroll 1
+    for (int q = 0; q < vt.nSTaps; ++q) {
+        const uint4 e = reinterpret_cast<const uint4 *>(f.HOT()->staps)[q];
+        a0 = fma(u2d(e.x, e.y), w[(int)e.z], a0);
+    }
+    return a0;
 }
 
 // ------------------------------------------------------------------------------------------ eval
@@ -388,10 +413,10 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
     double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, up = 0.0, dn = 0.0, bandR = 0.0;
     double *wtot = f.RED(), *eUp = f.RED() + 16, *eDn = f.RED() + 32;
     const double *wst = f.WST();
-    if (warp < nb) {
+    if (V3X_R && warp < nb) {
         const double *pp = reinterpret_cast<const double *>(f.base + vt.oROWP) + 96 * f.HOT()->rpBase[warp] + lane;
         const int np = f.HOT()->rpCnt[warp];
-#pragma unroll 4
+#pragma unroll 2
         for (int p = 0; p < np; ++p) {
             dm1 += pp[96 * p]; d0 += pp[96 * p + 32]; dp1 += pp[96 * p + 64];
         }
@@ -401,24 +426,21 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         up = __shfl_up_sync(0xffffffffu, dp1, 1);
         dn = __shfl_down_sync(0xffffffffu, dm1, 1);
         bandR = v3_taps(f, wst, min(k, N - 1), 0, vt.nTapsR);
-    } else if (warp < 2 * nb) {
+    } else if (V3X_C && warp >= nb && warp < 2 * nb) {
         const int g = warp - nb, kc = 32 * g + lane;
         const double2 *colp = reinterpret_cast<const double2 *>(f.base + vt.oCOLP);
         auto colsum = [&](int j, double &gj, double &hj) {
             const int c = j >> 5, np = f.HOT()->cpCnt[c];
             const double2 *pc2 = colp + 32 * f.HOT()->cpBase[c] + (j & 31);
             gj = 0.0; hj = 0.0;
-#pragma unroll 4
+#pragma unroll 2
             for (int r = 0; r < np; ++r) {
                 const double2 u = pc2[32 * r];
                 gj += u.x; hj += u.y;
             }
         };
-        double sl = 0.0;
-        {   // S stencil of l-bin kc (stage entries past the bins are 0) and its exceptions
-#pragma unroll 1
-            for (int q = 0; q < vt.nSTaps; ++q) sl = fma(f.HOT()->staps[q].c, wst[f.HOT()->staps[q].off + min(kc, N - 1)], sl);
-        }
+        // S stencil of l-bin kc (stage entries past the bins are 0) and its exceptions
+        double sl = v3_staps(vt, f, wst, min(kc, N - 1));
         if (vt.nExcS) sl = v3_exceptions(f, wst, g, 1, lane, sl);
         if (kc < N) {
             const int2 bi = f.BINI()[kc];
@@ -440,7 +462,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         }
         if (lane == 0) wtot[g] = suf;
         if (kc < N) f.YY()[kc].y = suf;
-    } else if (warp < 3 * nb) {
+    } else if (V3X_D && warp >= 2 * nb && warp < 3 * nb) {
         const int g = warp - 2 * nb, t = 32 * g + lane;
         double da = v3_taps(f, wst, min(t, N - 1), vt.nTapsR, vt.nTaps);       // (the list is padded to a multiple of 8)
         if (!vt.excLocal) da = v3_exceptions(f, wst, g, 0, lane, da);
@@ -461,6 +483,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
     double d = 0.0;
     if (live) {
         double suf = f.YY()[k].y;
+#pragma unroll 1
         for (int w = warp + 1; w < nb; ++w) suf += wtot[w];
         const double prev = (lane > 0) ? up : (warp > 0 ? eUp[warp - 1] : 0.0);
         const double next = (lane < 31) ? dn : (warp + 1 < nb ? eDn[warp + 1] : 0.0);
@@ -567,6 +590,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     auto flush_err = [&]() {
         if (MODE == MODE_STEP && tid == 0 && err_cell >= 0) {
             unsigned long long m = 0ull;
+#pragma unroll 1
             for (int w = 0; w < nb; ++w) {
                 const unsigned long long v = reinterpret_cast<const unsigned long long *>(s.RED)[64 + w];
                 m = v > m ? v : m;
@@ -617,12 +641,9 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         take_gas();
         flush_err();
         // the role vectors are dead: zero the padding of the band stage (its bins are written per evaluation)
-        {
-            const int padB = vt.wRow - vt.wPad - N, npad = vt.wPad + padB, rows = 2 * vt.bandD;
-            for (int q = tid; q < rows * npad; q += NT) {
-                const int r = q / npad, e = q - r * npad;
-                f.WST()[r * vt.wRow + (e < vt.wPad ? e : N + e)] = 0.0;
-            }
+        {   // (16 threads per stage row; the host checks that this covers them)
+            const int r = tid >> 4, e = tid & 15;
+            if (r < 2 * vt.bandD && e < vt.wRow - N) f.WST()[r * vt.wRow + (e < vt.wPad ? e : N + e)] = 0.0;
         }
 
         const bool more = cell + (int)gridDim.x < sa.C;
@@ -661,6 +682,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         // errors are >= 0 or NaN, so the unsigned order of their bit patterns is the NaN-propagating max)
         if (warp < nb) {
             double ysum = 0.0;
+#pragma unroll 1
             for (int w = 0; w < nb; ++w) ysum += s.RED[48 + w];
             const double atol = sa.atol_factor * ysum;
             unsigned long long eb = 0ull;

@@ -90,7 +90,7 @@ V3_HD inline V3RowRun v3_unpack_row(uint32_t w)
     return r;
 }
 
-struct V3Tap {                         // target t += c * W[off + t]   (off = plane, d and -o folded, in doubles)
+struct alignas(16) V3Tap {             // target t += c * W[off + t]   (off = plane, d and -o folded, in doubles)
     double c;
     int off, pad;
 };
@@ -126,7 +126,7 @@ struct V3Tables {
     int wRow;                          // entries per (plane, d) row of the W stage; entry of bin i at wPad + i
     int wPad;
     int nTaps, nSTaps, nExc, nExcT;
-    int nTapsR;                        // taps [0, nTapsR) go to combine group R, the rest to group D (multiples of 4)
+    int nTapsR;                        // taps [0, nTapsR) go to combine group R, the rest to group D (multiples of 8)
     int nExcS;                         // exception entries of S targets (kind 1)
     int excLocal;                      // 1: every density exception reads stage entries of its target's own 32-bin block, so
                                        //    the warp that staged the block sums them right away (phase A)

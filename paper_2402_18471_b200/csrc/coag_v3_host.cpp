@@ -15,8 +15,8 @@ namespace {
 
 // cost model (cycles of one warp; measured ratios on B200, only the ratios matter)
 constexpr double kCBuildRow = 95.0, kCBuildFold = 120.0, kCBuildDiagCopy = 320.0, kCBuildOwnerLate = 250.0;
-constexpr double kCColChunk = 450.0, kCColRun = 150.0;
-constexpr double kCRowRect = 70.0, kCRowRag = 110.0, kCRowRun = 300.0;
+constexpr double kCColChunk = 600.0, kCColRun = 150.0;
+constexpr double kCRowRect = 64.0, kCRowRag = 85.0, kCRowRun = 300.0;
 constexpr double kCStage = 500.0;          // band stage of 32 bins (warps of combine group D)
 constexpr double kCProlPiece = 2900.0;     // a third of the next cell's prologue, on the bin-owning warps
 
@@ -67,6 +67,8 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
     t.wPad = (omax + 1) & ~1;
     t.wRow = (t.wPad + N + (-omin) + 1) & ~1;
     if (2 * D * t.wRow > 32000) { out.why = "band stage too large"; return; }
+    // the kernel zeroes the padding of the stage with 16 threads per (plane, d) row
+    if (t.wRow - N > 16 || 2 * D > 32 * kV3Warps / 16) { out.why = "band stage padding too wide"; return; }
     t.nTaps = t.nSTaps = 0;
     for (auto &kv : cc) {                          // sorted by (kind, d, plane, o): fixed summation order
         const Key &k = kv.first;
@@ -118,7 +120,7 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
         V3Tap z; z.c = 0.0; z.off = t.wPad; z.pad = 0;
         t.hot.taps[t.nTaps++] = z;
     }
-    t.nTapsR = (2 * t.nTaps / 5) & ~3;
+    t.nTapsR = (2 * t.nTaps / 5) & ~7;
     t.nExcS = 0; t.excLocal = 1;
     for (int q = 0; q < t.nExc; ++q) {
         const V3Exc &x = t.hot.exc[q];
