@@ -353,9 +353,8 @@ __device__ __forceinline__ double v3_staps(const V3Tables &vt, const VSm &f, con
 template <int NT>
 __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &vt, const VSm &f, double y,
                                           double c1, double c2, double c3, int tid, uint32_t tq, int ppart,
-                                          const CellGas &nx, double mu, double sigma_mol, ProlState &ps,
-                                          RoleVals &rv, const uint32_t (&colw)[kV3ColRuns],
-                                          const uint32_t (&roww)[kV3RowRuns], bool storeNext, double nvR, double nvZ)
+                                          const CellDerived &nd, const GasArgs &gs, bool deriveNext, ProlState &ps,
+                                          RoleVals &rv, bool storeNext, double nvR, double nvZ)
 {
     const int N = vt.N, nb = vt.nb;
     const int lane = tid & 31, warp = tid >> 5;
@@ -382,22 +381,25 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
             excA = v3_exceptions(f, f.WST(), warp, 0, lane, 0.0);
         }
         if (ppart) {
-            if (ppart == 1 || ppart == 4) ps = prologue_begin(tb, nx, mu, sigma_mol, k);
+            if (ppart == 1 || ppart == 4) ps = prologue_begin(tb, nd, k);
             prologue_newton(ps, ppart == 4 ? 6 : 2);
-            if (ppart >= 3) rv = prologue_finish(tb, nx, mu, ps, c2, k);
+            if (ppart >= 3) rv = prologue_finish(tb, nd, ps, c2, k);
         }
     }
     // (one copy of each run body: the instruction cache matters more than the select chain.  Column runs
-    //  first on every warp: starting odd warps on their row runs instead was measured slower)
+    //  first on every warp: starting odd warps on their row runs instead was measured slower.  The packed runs
+    //  are read here, not held in registers across the build.)
+    const uint4 colw = reinterpret_cast<const uint4 *>(f.base + kV3oRUNS)[2 * warp];
+    const uint4 roww = reinterpret_cast<const uint4 *>(f.base + kV3oRUNS)[2 * warp + 1];
 #pragma unroll 1
     for (int r = 0; r < kV3ColRuns; ++r) {
-        const uint32_t w = r == 0 ? colw[0] : (r == 1 ? colw[1] : (r == 2 ? colw[2] : colw[3]));
+        const uint32_t w = r == 0 ? colw.x : (r == 1 ? colw.y : (r == 2 ? colw.z : colw.w));
         if (!w) break;
         v3_col_run(vt, f, v3_unpack_col(w), tq, lane);
     }
 #pragma unroll 1
     for (int r = 0; r < kV3RowRuns; ++r) {
-        const uint32_t w = r == 0 ? roww[0] : (r == 1 ? roww[1] : roww[2]);
+        const uint32_t w = r == 0 ? roww.x : (r == 1 ? roww.y : roww.z);
         if (!w) break;
         v3_row_run(tb, vt, f, v3_unpack_row(w), lane);
     }
@@ -467,6 +469,14 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         double da = v3_taps(f, wst, min(t, N - 1), vt.nTapsR, vt.nTaps);       // (the list is padded to a multiple of 8)
         if (!vt.excLocal) da = v3_exceptions(f, wst, g, 0, lane, da);
         f.BANDV()[t] = da;
+    } else if (deriveNext && warp == kV3Warps - 1) {
+        // the warp with no part in the combine: the per-cell scalars of the cell after the next one (its gas
+        // values landed in RED[80 .. 83] with this cell's build), for the bin owners to pick up after the next build
+        const CellGas g = {f.RED()[80], f.RED()[81], f.RED()[82], gs.alpha ? f.RED()[83] : gs.alpha_const};
+        const CellDerived d = derive_cell(g, gs.mu, gs.sigma_mol);
+        if (lane == 0) {
+            f.RED()[84] = d.Ste; f.RED()[85] = d.den; f.RED()[86] = d.Om; f.RED()[87] = d.Vg2; f.RED()[88] = d.bmc;
+        }
     }
     __syncthreads();
     // last evaluation of a cell: the partial sums are consumed, so the role vectors of the NEXT cell go into the
@@ -525,12 +535,13 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     }
     for (int q = tid; q < (int)(sizeof(V3Hot) / 4); q += NT)
         reinterpret_cast<uint32_t *>(smem_v3 + kV3oHOT)[q] = reinterpret_cast<const uint32_t *>(&vt.hot)[q];
-    // the thread's runs (kernel parameters -> registers) and the constants of its role (v3_eval)
-    uint32_t colw[kV3ColRuns], roww[kV3RowRuns];
-#pragma unroll
-    for (int r = 0; r < kV3ColRuns; ++r) colw[r] = vt.col[warp][r];
-#pragma unroll
-    for (int r = 0; r < kV3RowRuns; ++r) roww[r] = vt.row[warp][r];
+    // the packed runs of every warp (kernel parameters -> shared memory) and the constants of the thread's role
+    // (v3_eval)
+    static_assert(kV3ColRuns == 4 && kV3RowRuns == 3, "run words: one uint4 of column runs, one of row runs per warp");
+    if (tid < 8 * kV3Warps) {
+        const int w = tid >> 3, r = tid & 7;
+        reinterpret_cast<uint32_t *>(smem_v3 + kV3oRUNS)[tid] = r < 4 ? vt.col[w][r] : (r < 7 ? vt.row[w][r - 4] : 0u);
+    }
     double c1 = 0.0, c2 = 0.0, c3 = 0.0;
     if (live) {
         c1 = tb.binc[BC_M * tb.Np + k]; c2 = tb.binc[BC_RM * tb.Np + k]; c3 = tb.binc[BC_FA * tb.Np + k];
@@ -557,30 +568,46 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     __syncthreads();
     tmem_fence_after();
 
-    // frozen inputs of a cell, fetched one cell ahead: the per-cell scalars at the
-    // start of the previous cell (its evaluations run the next prologue piece by piece), the per-bin
-    // velocities two evaluations before its end
-    CellGas nx = {1.0, 1.0, 1.0, 1.0};
+    // frozen inputs of a cell, fetched ahead: the per-cell scalars two cells ahead (the warp
+    // that idles in the combine phase turns them into what the prologue needs, RED[84 .. 88], and the evaluations
+    // of the cell before run that prologue piece by piece), the per-bin velocities two evaluations before the
+    // end of the cell before
+    CellDerived nd = {1.0, 1.0, 1.0, 1.0, 1.0};
     double nvR = 0.0, nvZ = 0.0;
     auto stage_gas = [&](int cell) {        // cp.async of the per-cell scalars into RED[80 .. 83]
         if (cell >= sa.C || tid >= 4) return;
         const double *src = tid == 0 ? gs.T : (tid == 1 ? gs.rho_g : (tid == 2 ? gs.Omega : gs.alpha));
         if (src) cp_async8(s.RED + 80 + tid, src + cell);
     };
-    auto take_gas = [&]() {
-        nx.T = s.RED[80]; nx.rho_g = s.RED[81]; nx.Om = s.RED[82];
-        nx.alpha = gs.alpha ? s.RED[83] : gs.alpha_const;
+    auto raw_gas = [&]() {
+        const CellGas g = {s.RED[80], s.RED[81], s.RED[82], gs.alpha ? s.RED[83] : gs.alpha_const};
+        return g;
+    };
+    auto take_derived = [&]() {
+        nd.Ste = s.RED[84]; nd.den = s.RED[85]; nd.Om = s.RED[86]; nd.Vg2 = s.RED[87]; nd.bmc = s.RED[88];
     };
     auto fetch_vel = [&](int cell) {
         if (cell >= sa.C || !live) return;
         const size_t g = (size_t)cell * N + k;
         nvR = __ldg(gs.vR + g); nvZ = __ldg(gs.vZ + g);
     };
+    // first cell of the CTA: nothing ran ahead, every thread takes the raw values; second cell: its scalars are
+    // derived here (once per launch)
     stage_gas(blockIdx.x);
     cp_async_wait_all();
     __syncthreads();
-    take_gas();
+    const CellGas g0 = raw_gas();
     fetch_vel(blockIdx.x);
+    __syncthreads();
+    stage_gas(blockIdx.x + gridDim.x);
+    cp_async_wait_all();
+    __syncthreads();
+    if (warp == kV3Warps - 1 && (int)(blockIdx.x + gridDim.x) < sa.C) {
+        const CellDerived d = derive_cell(raw_gas(), gs.mu, gs.sigma_mol);
+        if (lane == 0) {
+            s.RED[84] = d.Ste; s.RED[85] = d.den; s.RED[86] = d.Om; s.RED[87] = d.Vg2; s.RED[88] = d.bmc;
+        }
+    }
     RoleVals rv;
     rv.Vg2 = 0.0;
     ProlState ps = {2.0, 0.0, 0.0, 0.0};
@@ -588,7 +615,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
 
     int err_cell = -1;          // cell whose warp error maxima wait in RED[64 ..) for the next barrier
     auto flush_err = [&]() {
-        if (MODE == MODE_STEP && tid == 0 && err_cell >= 0) {
+        if (MODE == MODE_STEP && tid == NT - 32 && err_cell >= 0) {     // (a thread of the warp that owns no bins)
             unsigned long long m = 0ull;
 #pragma unroll 1
             for (int w = 0; w < nb; ++w) {
@@ -601,7 +628,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
         const size_t row = (size_t)cell * N;
         if (!rv_valid) {                              // first cell of the CTA: nothing ran ahead
-            rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, c2, k);
+            rv = prologue_compute(tb, g0, gs.mu, gs.sigma_mol, c2, k);
             prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
             if (tid == 0) s.RED[95] = rv.Vg2;
             __syncthreads();
@@ -613,10 +640,10 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             cp_async8(&f.YY()[k].x, sa.rho + row + k);
             if (MODE == MODE_STEP && sa.have_k1) cp_async8(&f.YY()[k].y, sa.k_fsal + row + k);
         }
-        stage_gas(cell + gridDim.x);
+        stage_gas(cell + 2 * gridDim.x);
 #pragma unroll 1
         for (int r = 0; r < kV3ColRuns; ++r) {
-            const uint32_t w = r == 0 ? colw[0] : (r == 1 ? colw[1] : (r == 2 ? colw[2] : colw[3]));
+            const uint32_t w = reinterpret_cast<const uint32_t *>(smem_v3 + kV3oRUNS)[8 * warp + r];
             if (!w) break;
             const V3ColRun run = v3_unpack_col(w);
             if (run.diag) v3_build_diag(vt, f, pc, run, tq, lane);
@@ -638,7 +665,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         tmem_fence_before();
         __syncthreads();
         tmem_fence_after();
-        take_gas();
+        take_derived();
         flush_err();
         // the role vectors are dead: zero the padding of the band stage (its bins are written per evaluation)
         {   // (16 threads per stage row; the host checks that this covers them)
@@ -646,11 +673,11 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             if (r < 2 * vt.bandD && e < vt.wRow - N) f.WST()[r * vt.wRow + (e < vt.wPad ? e : N + e)] = 0.0;
         }
 
-        const bool more = cell + (int)gridDim.x < sa.C;
+        const bool more = cell + (int)gridDim.x < sa.C, more2 = cell + 2 * (int)gridDim.x < sa.C;
         if (MODE == MODE_OTF) {
             fetch_vel(cell + gridDim.x);
-            const double d = v3_eval<NT>(tb, vt, f, y0, c1, c2, c3, tid, tq, more ? 4 : 0, nx, gs.mu,
-                                         gs.sigma_mol, ps, rv, colw, roww, more, nvR, nvZ);
+            const double d = v3_eval<NT>(tb, vt, f, y0, c1, c2, c3, tid, tq, more ? 4 : 0, nd, gs, more2, ps, rv,
+                                         more, nvR, nvZ);
             rv_valid = more;
             if (live) sa.out[row + k] = d;
             continue;
@@ -669,8 +696,8 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
                 yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
                 ys = yn;
             }
-            const double d = v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nx, gs.mu,
-                                         gs.sigma_mol, ps, rv, colw, roww, more && st == 3, nvR, nvZ);
+            const double d = v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nd, gs, more2 && st == 1,
+                                         ps, rv, more && st == 3, nvR, nvZ);
             if (st == 3) rv_valid = more;
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;

@@ -10,8 +10,8 @@
 // A warp reaches only the tensor-memory lanes of its quarter (warp % 4), so a chunk is built and later
 // summed by the same warp.  All work of a cell is dealt out STATICALLY on the host (this file's V3Tables,
 // passed to the kernel by value): per warp a few "runs" of column chunks and of row-pass columns, packed
-// one run per 32-bit word and decoded once per launch into registers.  No queues, no atomics, fixed
-// summation order.
+// one run per 32-bit word, copied to shared memory once per launch and decoded where a phase starts.  No queues,
+// no atomics, fixed summation order.
 //
 // Band as a stencil.  coag_tables.cpp lists every outcome that the bulk row / column sums do not cover as
 // gather entries (target, i, j, plane, coef).  On a grid with constant mass ratio coef / m_i depends only on
@@ -52,7 +52,8 @@ constexpr int kV3oNN = kV3oYY + 16 * kV3NpMax;               // double[160 + 16]
 constexpr int kV3oBANDV = kV3oNN + 8 * (kV3NpMax + 16);      // double[160]  band sums of the density targets
 constexpr int kV3oHOT = kV3oBANDV + 8 * kV3NpMax;            // V3Hot: the small tables the loops index (copied from the parameters)
 constexpr int kV3HotBytes = 1600;
-constexpr int kV3oUNION = kV3oHOT + kV3HotBytes;             // build: role vectors; evaluation: W stage, partial sums
+constexpr int kV3oRUNS = kV3oHOT + kV3HotBytes;              // uint32[16][8]: the packed runs of every warp (4 column, 3 row, 1 unused)
+constexpr int kV3oUNION = kV3oRUNS + 32 * kV3Warps;          // build: role vectors; evaluation: W stage, partial sums
 constexpr int kV3BuildUnionBytes = 8 * 19 * kV3NpMax;
 constexpr int kV3ColSlotBytes = 32 * 16;                     // (G, H) per lane
 constexpr int kV3RowSlotBytes = 32 * 24;                     // deposits into bins i-1, i, i+1 (per unit n_i), [3][32]
