@@ -8,24 +8,18 @@
 //     tensor memory (tcgen05.st, lane <-> column j, 8-row chunks); a 32 x 32 diagonal block is built with
 //     its short and long rows folded into full warps, then copied to tensor memory with zeros above the
 //     diagonal;
-//   * a rate evaluation reads the row copy once (row pass) and the column copy once (column pass,
-//     tcgen05.ld, the next half chunk in flight while the current one is summed);
+//   * a rate evaluation reads the row copy once (row pass) and the column copy once (column pass, one
+//     tcgen05.ld of 8 rows per chunk);
 //   * the near-diagonal outcomes are a stencil over the staged products y_i n_{i-d} K[i][i-d] with
-//     warp-uniform coefficients from the constant bank (+ a few exception entries at the grid ends);
-//   * every warp owns a static list of runs (kernel parameter V3Tables, decoded into registers once): no
-//     queues, no atomics, fixed summation order -> results are bit-reproducible.
+//     warp-uniform coefficients from a small table in shared memory (+ a few exception entries at the grid
+//     ends);
+//   * every warp owns a static list of runs (kernel parameter V3Tables, copied to shared memory once per
+//     launch): no queues, no atomics, fixed summation order -> results are bit-reproducible;
+//   * nothing that is the same for every bin runs between two block barriers: the per-cell scalars of the
+//     prologue are derived two cells ahead by the warp that has no part in the combine phase.
 // One persistent CTA of 512 threads per SM; thread k < N owns bin k (state and derivatives in registers).
 #include "coag_v3.h"
 #include "coag_launch.h"
-#ifndef V3X_R
-#define V3X_R 1
-#endif
-#ifndef V3X_C
-#define V3X_C 1
-#endif
-#ifndef V3X_D
-#define V3X_D 1
-#endif
 
 namespace cudisc {
 
@@ -415,7 +409,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
     double d0 = 0.0, dm1 = 0.0, dp1 = 0.0, up = 0.0, dn = 0.0, bandR = 0.0;
     double *wtot = f.RED(), *eUp = f.RED() + 16, *eDn = f.RED() + 32;
     const double *wst = f.WST();
-    if (V3X_R && warp < nb) {
+    if (warp < nb) {
         const double *pp = reinterpret_cast<const double *>(f.base + vt.oROWP) + 96 * f.HOT()->rpBase[warp] + lane;
         const int np = f.HOT()->rpCnt[warp];
 #pragma unroll 2
@@ -428,7 +422,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         up = __shfl_up_sync(0xffffffffu, dp1, 1);
         dn = __shfl_down_sync(0xffffffffu, dm1, 1);
         bandR = v3_taps(f, wst, min(k, N - 1), 0, vt.nTapsR);
-    } else if (V3X_C && warp >= nb && warp < 2 * nb) {
+    } else if (warp < 2 * nb) {
         const int g = warp - nb, kc = 32 * g + lane;
         const double2 *colp = reinterpret_cast<const double2 *>(f.base + vt.oCOLP);
         auto colsum = [&](int j, double &gj, double &hj) {
@@ -464,7 +458,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         }
         if (lane == 0) wtot[g] = suf;
         if (kc < N) f.YY()[kc].y = suf;
-    } else if (V3X_D && warp >= 2 * nb && warp < 3 * nb) {
+    } else if (warp < 3 * nb) {
         const int g = warp - 2 * nb, t = 32 * g + lane;
         double da = v3_taps(f, wst, min(t, N - 1), vt.nTapsR, vt.nTaps);       // (the list is padded to a multiple of 8)
         if (!vt.excLocal) da = v3_exceptions(f, wst, g, 0, lane, da);

@@ -18,8 +18,8 @@
 // (d = i - j, o = target - i, plane, kind) away from the grid ends.  Per evaluation one warp group
 // stages  W[plane][d][i] = y_i n_{i-d} Kplane[i][i-d]   (y_i = m_i n_i; d < bandD) in shared memory, and
 //   dens[t] = sum_taps c W[plane][d][t - o],   S[t] likewise,
-// with warp-uniform coefficients from the constant bank, plus a short list of exception entries at the grid
-// ends that carries the residual coefficients.  The host re-expands taps + exceptions and checks them against
+// with warp-uniform coefficients from a small table in shared memory (one 16-byte entry per tap), plus a short
+// list of exception entries at the grid ends that carries the residual coefficients.  The host re-expands taps + exceptions and checks them against
 // the gather entries (v3_build refuses the grid otherwise; v3_check re-evaluates both on pseudo-random
 // data), so the stencil is a restatement of the table, not an approximation of it.
 #pragma once
