@@ -314,7 +314,7 @@ def run_ours(args):
                 "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops,
                 # dram__bytes_read.sum + dram__bytes_write.sum of one launch (ncu --set full), profiles/r02_kernels.md
-                "traffic": 194343680 if (args.config == 4 and world == 1) else
+                "traffic": 193767936 if (args.config == 4 and world == 1) else
                            (1226387200 if (args.config == 5 and world == 1) else None),
                 "how": f"algorithmic FP64 instructions per launch = C*P*({I_BUILD} + {EVALS_PER_STEP}*{I_EVAL}) "
                        f"= {alg_instr:.4g} (DESIGN.md 'Roofline'), x2 flop per FP64 issue slot, / mean CUDA-event "
@@ -326,8 +326,8 @@ def run_ours(args):
                 "hbm_algorithmic_gbs": (6.0 * C * N * 8 + 5.0 * C * 8) / kernel_s / 1e9,
                 "note": "the FP64 pipe is the roofline BASELINE.json names; frac is the share of FP64 issue slots the "
                         "algorithmic instructions would need, not a FLOP/s claim.  ncu (profiles/r02_kernels.md): the "
-                        "kernel is latency-bound (16 warps per SM, issue slots 48 %, FP64 pipe 28 %, shared-memory pipe "
-                        "49 %), see DESIGN.md 'Roofline'",
+                        "kernel is latency-bound (16 warps per SM, issue slots 53 %, FP64 pipe 31 %, shared-memory pipe "
+                        "58 %), see DESIGN.md 'Roofline'",
             },
         }
         if world == 1 and not args.no_cpu_baseline:
