@@ -183,6 +183,25 @@ int cudisc_coag_rates(cudisc_grid g, cudisc_bins b, const double *K,
 int cudisc_coag_rates_otf(cudisc_grid g, cudisc_bins b, const double *rho_dust, double *drho_dt,
                           cudisc_stream stream);
 
+/* cudisc_coag_rates_otf for callers that may not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same operation, same arguments, same results, on the general cell
+ * kernel (coag_kernels.cu), whose scratch -- the per-CTA slab for the pairs of K that do not fit in shared
+ * memory, (P - P_shared) x 16 B per resident CTA -- lives in a file-scope device array of the library instead
+ * of the grid's own buffer.  The call performs no cudaMalloc / cudaFree and calls no allocating library
+ * routine; g and b must exist already (cudisc_grid_create uploads the tables), and the first call on a device
+ * looks the array's address up (cudaGetSymbolAddress: no allocation), so make one call at set-up.
+ * Limit: the array holds CUDISC_STATIC_SCRATCH_BYTES = 24 MiB on every GPU that loads the library, until
+ * the process exits: enough for every grid of up to 200 bins on a 148-SM GPU (21.7 MiB); a grid that needs more
+ * is rejected with CUDISC_ERR_UNSUPPORTED and a message that states both sizes (use cudisc_coag_rates_otf).
+ * Grids whose K fits in shared memory use no scratch at all.
+ * All calls share the array and it keeps the last call's contents; the kernel writes every slab entry of a
+ * cell before reading it, so nothing needs clearing -- but two calls of this entry point that OVERLAP on
+ * the GPU (different streams, or graph branches) race on it: serialise them.
+ * rho_dust: DEVICE [C x N] in; drho_dt: DEVICE [C x N] out.  May not alias. */
+#define CUDISC_STATIC_SCRATCH_BYTES (24u << 20)
+int cudisc_coag_rates_otf_noalloc(cudisc_grid g, cudisc_bins b, const double *rho_dust, double *drho_dt,
+                                  cudisc_stream stream);
+
 /* One Bogacki-Shampine 3(2) step of size dt (s) of every cell, with the kernel
  * built on the fly, once per cell per step, from the gas state bound to g and frozen over the
  * stages; parameters are those given to cudisc_bins_create.

@@ -45,6 +45,7 @@ EXPORTS = [
     "cudisc_bins_create", "cudisc_bins_create_general", "cudisc_bins_destroy", "cudisc_bins_query",
     "cudisc_bins_expand_outcomes", "cudisc_bins_schedule_check", "cudisc_bins_fast_path", "cudisc_grid_create", "cudisc_grid_bind_gas", "cudisc_grid_reset_fsal",
     "cudisc_grid_destroy", "cudisc_coag_kernel", "cudisc_coag_rates", "cudisc_coag_rates_otf",
+    "cudisc_coag_rates_otf_noalloc",
     "cudisc_coag_step", "cudisc_coag_step_cached", "cudisc_coag_step_host", "cudisc_coag_integrate", "cudisc_coag_integrate_steps", "cudisc_controller_next_dt",
     "cudisc_microbench_dfma",
     "cudisc_microbench_copy", "cudisc_launch_count", "cudisc_last_error", "cudisc_version",
@@ -77,6 +78,7 @@ def lib() -> C.CDLL:
         L.cudisc_coag_kernel.argtypes = [vp, vp, C.POINTER(cudisc_gas_state), cudisc_params, vp, vp]
         L.cudisc_coag_rates.argtypes = [vp, vp, vp, vp, vp, vp]
         L.cudisc_coag_rates_otf.argtypes = [vp, vp, vp, vp, vp]
+        L.cudisc_coag_rates_otf_noalloc.argtypes = [vp, vp, vp, vp, vp]
         L.cudisc_coag_step.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.cudisc_coag_step_host.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.cudisc_coag_step_cached.argtypes = [vp, vp, vp, vp, C.c_double, vp, vp]
@@ -277,6 +279,16 @@ def cudisc_coag_rates_otf(grid: Grid, bins: Bins, rho_dust, drho_dt, stream=None
     Cn, N = grid.n_cells, bins.n_bins
     _check(lib().cudisc_coag_rates_otf(grid.handle, bins.handle, _dev_ptr(rho_dust, "rho_dust", Cn * N),
                                        _dev_ptr(drho_dt, "drho_dt", Cn * N), _stream(stream)))
+
+
+STATIC_SCRATCH_BYTES = 24 << 20     # CUDISC_STATIC_SCRATCH_BYTES of include/cudisc_coag.h
+
+
+def cudisc_coag_rates_otf_noalloc(grid: Grid, bins: Bins, rho_dust, drho_dt, stream=None) -> None:
+    """cudisc_coag_rates_otf without any allocation: the kernel's scratch is the library's static device array."""
+    Cn, N = grid.n_cells, bins.n_bins
+    _check(lib().cudisc_coag_rates_otf_noalloc(grid.handle, bins.handle, _dev_ptr(rho_dust, "rho_dust", Cn * N),
+                                               _dev_ptr(drho_dt, "drho_dt", Cn * N), _stream(stream)))
 
 
 def cudisc_coag_step(grid: Grid, bins: Bins, rho_dust, dt: float, err_out, stream=None) -> None:

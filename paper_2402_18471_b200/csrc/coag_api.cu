@@ -786,6 +786,40 @@ int cudisc_coag_rates_otf(cudisc_grid g, cudisc_bins b, const double *rho_dust, 
     return run(g, 2, gas_args(g->gs, b->p), sa, stream);
 }
 
+int cudisc_coag_rates_otf_noalloc(cudisc_grid g, cudisc_bins b, const double *rho_dust, double *drho_dt,
+                                  cudisc_stream stream)
+{
+    static_assert(kStaticSlabBytes == CUDISC_STATIC_SCRATCH_BYTES, "header and kernel file disagree on the scratch size");
+    int rc = check_pair(g, b);
+    if (rc) return rc;
+    if (!g->gas_bound) return fail(CUDISC_ERR_INVALID, "no gas state bound (cudisc_grid_bind_gas)");
+    if (!rho_dust || !drho_dt) return fail(CUDISC_ERR_INVALID, "NULL array argument");
+    if (rho_dust == drho_dt) return fail(CUDISC_ERR_INVALID, "rho_dust and drho_dt may not alias");
+    // nothing on this path may allocate: the tables must be on the current device already
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (!b->on_device || b->device != dev)
+        return fail(CUDISC_ERR_INVALID, "tables of this mass grid are not on the current device (create the grid there first)");
+    const DevTables &d = b->dt;
+    const int ctas = std::min(g->grid_ctas, std::max(1, g->C));
+    const size_t need = d.P > g->Psm ? (size_t)ctas * (size_t)(d.P - g->Psm) * 16 : 0;
+    if (need > kStaticSlabBytes)
+        return fail(CUDISC_ERR_UNSUPPORTED,
+                    "n_bins %d on %d CTAs needs %zu B of scratch, the static array holds %zu B: use cudisc_coag_rates_otf",
+                    d.N, ctas, need, (size_t)kStaticSlabBytes);
+    StepArgs sa;
+    memset(&sa, 0, sizeof(sa));
+    sa.rho = rho_dust; sa.out = drho_dt;
+    sa.C = g->C;
+    sa.Psm = g->Psm;
+    LaunchCfg lc{ctas, g->smem_bytes, g->smem_optin};
+    e = launch_cells_static_slab(MODE_OTF, lc, d, gas_args(g->gs, b->p), sa, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "kernel launch (static scratch)");
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CUDISC_OK;
+}
+
 int cudisc_coag_step(cudisc_grid g, cudisc_bins b, double *rho_dust, double dt, double *err_out,
                      cudisc_stream stream)
 {

@@ -749,4 +749,32 @@ cudaError_t launch_copy_peak(int grid, const void *src, void *dst, size_t n16, c
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------ static scratch
+// The per-CTA overflow slab of the K store for callers that may not allocate (cudisc_coag_rates_otf_noalloc):
+// a file-scope array, so every GPU that loads the library holds kStaticSlabBytes of it until the process exits.
+// In host code `g_static_slab` is only a stand-in for the symbol, not a device address: the address comes from
+// cudaGetSymbolAddress, looked up once per device with that device current, and goes to the kernel in
+// StepArgs::kslab.  All calls share the array; the kernel writes every slab pair of a cell before it reads it,
+// so nothing has to be cleared between calls -- but two launches that overlap on the GPU would race on it.
+static __device__ __align__(256) unsigned char g_static_slab[kStaticSlabBytes];
+
+cudaError_t launch_cells_static_slab(int mode, const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
+                                     const StepArgs &sa_in, cudaStream_t st)
+{
+    static void *addr[64] = {nullptr};      // per device
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!addr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_slab);
+        if (e != cudaSuccess) return e;
+        addr[dev] = p;
+    }
+    StepArgs sa = sa_in;
+    sa.kslab = reinterpret_cast<double *>(addr[dev]);
+    return launch_cells(mode, lc, tb, gs, sa, st);
+}
+
 }  // namespace cudisc

@@ -18,6 +18,11 @@ struct LaunchCfg {
 // mode: 0 kernel, 1 rates (supplied K), 2 rates on the fly, 3 BS3(2) step
 cudaError_t launch_cells(int mode, const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
                          const StepArgs &sa, cudaStream_t st);
+// launch_cells with the K-overflow slab in the library's file-scope scratch array instead of sa.kslab (no
+// allocation anywhere on this path); the caller has checked lc.grid * (P - Psm) * 16 <= kStaticSlabBytes
+constexpr size_t kStaticSlabBytes = (size_t)24 << 20;
+cudaError_t launch_cells_static_slab(int mode, const LaunchCfg &lc, const DevTables &tb, const GasArgs &gs,
+                                     const StepArgs &sa, cudaStream_t st);
 // the stencil cell kernel (coag_v3.cu): MODE_OTF or MODE_STEP on a mass grid with vt.on
 struct V3Tables;
 cudaError_t launch_v3(int mode, const LaunchCfg &lc, const DevTables &tb, const V3Tables &vt,
