@@ -93,11 +93,49 @@ __device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, c
 // ------------------------------------------------------------------------------------------ eval
 // One rate evaluation of the current cell: thread k < N passes y_k and gets drho_k/dt.
 // Three block barriers; every partial sum has its own slot and every combination a fixed order.
-template <int NT, bool SLAB>
-__device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s, const KStore<SLAB> &ks,
+// Asynchronous refill of a PLANAR K store from the planes of a cell: 1-D bulk copies (TMA) of the 16 P bytes,
+// completing on an mbarrier.  Called by one thread, after a block barrier behind the last read of the old contents.
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void refill_bulk(void *ksm, const double *planes, int P, uint64_t *bar)
+{
+    const uint32_t bytes = 16u * (uint32_t)P;
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" :: "r"(smem_addr(bar)), "r"(bytes) : "memory");
+    constexpr uint32_t kChunk = 32768;
+    for (uint32_t off = 0; off < bytes; off += kChunk) {
+        const uint32_t n = bytes - off < kChunk ? bytes - off : kChunk;
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                     :: "r"(smem_addr(ksm) + off), "l"(reinterpret_cast<const char *>(planes) + off), "r"(n),
+                        "r"(smem_addr(bar)) : "memory");
+    }
+}
+__device__ __forceinline__ void mbar_wait_parity(uint64_t *bar, uint32_t parity)
+{
+    asm volatile("{\n.reg .pred p;\nWAIT_%=:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@!p bra WAIT_%=;\n}\n" :: "r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+constexpr int kRedMbar = 88;     // Smem::RED slot that holds the mbarrier of the refill
+
+// The same for a store of (Kc, Kf) pairs (cudisc_coag_step_cached: three evaluations per load, and the pair layout
+// makes an evaluation 20 % faster than the planar one): 8-byte LDGSTS copies, plane 0 -> .x, plane 1 -> .y of
+// every pair, by all threads; completed by cp.async.wait_all + a block barrier.
+__device__ __forceinline__ void refill_pairs(double2 *ksm, const double *planes, int P, int tid, int nt)
+{
+    for (int p = tid; p < P; p += nt) {
+        const uint32_t dst = smem_addr(ksm + p);
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" :: "r"(dst), "l"(planes + p) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" :: "r"(dst + 8), "l"(planes + P + p) : "memory");
+    }
+}
+
+// kin_next: planes of the cell whose kernel the K store takes NEXT (modes that read K from HBM, last evaluation of
+// a cell), or nullptr: the refill starts as soon as the last read of K is behind the block, under the combine phase.
+template <int NT, bool SLAB, bool PLANAR>
+__device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s, const KStore<SLAB, PLANAR> &ks,
                                              double y, int tid, uint32_t tbase,
                                              bool pre, const CellGas &nx, double mu, double sigma_mol,
-                                             RoleVals &rv)
+                                             RoleVals &rv, const double *kin_next = nullptr)
 {
     const int N = tb.N, Np = tb.Np;
     const int lane = tid & 31, warp = tid >> 5;
@@ -144,7 +182,8 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
                 for (int u = 0; u < 8; ++u) {
                     const int i = ixs[u] & 0xff, j = (ixs[u] >> 8) & 0xff;
                     const int p2 = 2 * (tri(i) + j) + (int)((ixs[u] >> 16) & 1);
-                    const double kv = SLAB ? ((ixs[u] >> 16) & 1 ? ks.ld(p2 >> 1).y : ks.ld(p2 >> 1).x) : kd[p2];
+                    const double kv = SLAB ? ((ixs[u] >> 16) & 1 ? ks.ld(p2 >> 1).y : ks.ld(p2 >> 1).x)
+                                           : (PLANAR ? kd[(p2 & 1) * tb.P + (p2 >> 1)] : kd[p2]);
                     const double c = __hiloint2double((int)cf[2 * u + 1], (int)cf[2 * u]);
                     if (u & 1) acc1 = fma(c * s.NN[i], s.NN[j] * kv, acc1);
                     else acc0 = fma(c * s.NN[i], s.NN[j] * kv, acc0);
@@ -283,6 +322,13 @@ __device__ __forceinline__ double eval_rates(const DevTables &tb, const Smem &s,
     }
     if (!band_done) band_from_stage();
     __syncthreads();
+    if (kin_next) {
+        if (PLANAR) {
+            if (tid == 0) refill_bulk(ks.sm, kin_next, tb.P, reinterpret_cast<uint64_t *>(s.RED + kRedMbar));
+        } else if (!SLAB) {
+            refill_pairs(ks.sm, kin_next, tb.P, tid, NT);
+        }
+    }
 
     // ---- phase B: combine partials in fixed order.  Two warp groups work side by side:
     //   group R (thread k, bin k)            row partials -> deposits into bins k-1, k, k+1
@@ -381,9 +427,11 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
     extern __shared__ __align__(16) double smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int N = tb.N, P = tb.P;
-    KStore<SLAB> ks;
+    constexpr bool PLANAR = MODE == MODE_RATES && !SLAB;
+    KStore<SLAB, PLANAR> ks;
     ks.sm = reinterpret_cast<double2 *>(smem_raw);
     ks.Psm = sa.Psm;
+    ks.P = P;
     ks.gl = reinterpret_cast<double2 *>(sa.kslab) + (size_t)blockIdx.x * (size_t)(P - sa.Psm);
     const Smem s = carve(smem_raw + 2 * (size_t)sa.Psm, tb.Np, tb.partRowSlots, tb.partColSlots,
                          tb.nBuildItems, tb.nEvalItems, tb.bandD);
@@ -464,6 +512,17 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
         }
     };
     fetch(blockIdx.x);
+    // refill of a PLANAR K store by bulk copies: mbarrier in RED, phase bit per cell
+    uint64_t *kbar = reinterpret_cast<uint64_t *>(s.RED + kRedMbar);
+    uint32_t kph = 0u;
+    const bool kin_tma = PLANAR && (reinterpret_cast<uintptr_t>(sa.Kin) & 15) == 0;
+    if (PLANAR) {
+        if (tid == 0) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" :: "r"(smem_addr(kbar)), "r"(1) : "memory");
+            asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        }
+        __syncthreads();
+    }
     RoleVals rv;
     rv.Vg2 = 0.0;
     bool rv_valid = false;       // rv holds the next cell's values (computed during the last evaluation)
@@ -473,21 +532,39 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
 
         // ---------------- K store for this cell
         if (MODE == MODE_RATES || MODE == MODE_STEPK) {
-            // flat, coalesced copy of both planes (8 loads in flight per thread), then the N diagonal
-            // entries are halved in place
+            // The planes of this cell.  Everything fits in shared memory: the refill that the CTA started behind the
+            // last read of its previous cell's kernel, i.e. under that cell's combine phase (eval_rates), lands here --
+            // bulk copies completing on the mbarrier (PLANAR store; planes that are not 16-byte aligned take a plain
+            // copy) or LDGSTS copies (store of pairs).  Slab: a flat, coalesced copy of both planes, 16 loads in
+            // flight per thread.
+            // Then the N diagonal entries are halved in place.
             const double *k0 = sa.Kin + (size_t)cell * 2 * P, *k1 = k0 + P;
-            for (int p0 = tid; p0 < P; p0 += 4 * NT) {
-                double a[4], b[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int p = p0 + u * NT;
-                    a[u] = p < P ? __ldcs(k0 + p) : 0.0;
-                    b[u] = p < P ? __ldcs(k1 + p) : 0.0;
+            if (PLANAR) {
+                if (kin_tma) {
+                    if (cell == (int)blockIdx.x && tid == 0) refill_bulk(ks.sm, k0, P, kbar);
+                    mbar_wait_parity(kbar, kph);
+                    kph ^= 1u;
+                } else {
+                    double *dstp = reinterpret_cast<double *>(ks.sm);
+                    for (int p = tid; p < 2 * P; p += NT) dstp[p] = __ldcs(k0 + p);
                 }
+            } else if (!SLAB) {
+                if (cell == (int)blockIdx.x) refill_pairs(ks.sm, k0, P, tid, NT);
+                asm volatile("cp.async.wait_all;\n" ::: "memory");
+            } else {
+                for (int p0 = tid; p0 < P; p0 += 8 * NT) {
+                    double a[8], b[8];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int p = p0 + u * NT;
-                    if (p < P) ks.st(p, make_double2(a[u], b[u]));
+                    for (int u = 0; u < 8; ++u) {
+                        const int p = p0 + u * NT;
+                        a[u] = p < P ? __ldcs(k0 + p) : 0.0;
+                        b[u] = p < P ? __ldcs(k1 + p) : 0.0;
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int p = p0 + u * NT;
+                        if (p < P) ks.st(p, make_double2(a[u], b[u]));
+                    }
                 }
             }
             __syncthreads();
@@ -495,6 +572,18 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
                 const int p = tri(k) + k;
                 const double2 v = ks.ld(p);
                 ks.st(p, make_double2(0.5 * v.x, 0.5 * v.y));
+            }
+            // The K store of a cell fills the shared memory, so the next cell's planes cannot be staged there while
+            // this one is evaluated: they are pulled into L2 meanwhile (asynchronous bulk prefetch, 8 KB per thread), and
+            // the refill then reads them at L2 speed.  In flight over the chip: one cell per CTA (27 MB at 150 bins).
+            if (cell + (int)gridDim.x < sa.C && (reinterpret_cast<uintptr_t>(sa.Kin) & 15) == 0) {
+                const char *nxt = reinterpret_cast<const char *>(sa.Kin + (size_t)(cell + gridDim.x) * 2 * P);
+                const size_t bytes = 16 * (size_t)P;
+                constexpr size_t kChunk = 8192;
+                for (size_t off = (size_t)tid * kChunk; off < bytes; off += (size_t)NT * kChunk) {
+                    const uint32_t n = (uint32_t)(bytes - off < kChunk ? bytes - off : kChunk);
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(nxt + off), "r"(n) : "memory");
+                }
             }
         } else {
             if (!rv_valid) rv = prologue_compute(tb, nx, gs.mu, gs.sigma_mol, live ? s.BINC[BC_RM * tb.Np + k] : 0.0, k);
@@ -510,7 +599,7 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
             y0 = sa.rho[row + k];
             if ((MODE == MODE_STEP || MODE == MODE_STEPK) && sa.have_k1) k1 = sa.k_fsal[row + k];
         }
-        if (MODE != MODE_RATES && MODE != MODE_STEPK)
+        if constexpr (MODE != MODE_RATES && MODE != MODE_STEPK)
             build_cell<MODE, SLAB>(tb, s, ks, pc, has_vphi,
                                    MODE == MODE_KERNEL ? sa.out + (size_t)cell * 2 * P : nullptr, lane);
         if (MODE == MODE_KERNEL) fetch(cell + gridDim.x);
@@ -538,7 +627,9 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
 
         if (MODE == MODE_RATES || MODE == MODE_OTF) {
             fetch(cell + gridDim.x);
-            const double d = eval_rates<NT, SLAB>(tb, s, ks, y0, tid, tbase, false, nx, gs.mu, gs.sigma_mol, rv);
+            const double *kn = (MODE == MODE_RATES && kin_tma && cell + (int)gridDim.x < sa.C)
+                                   ? sa.Kin + (size_t)(cell + gridDim.x) * 2 * P : nullptr;
+            const double d = eval_rates<NT, SLAB, PLANAR>(tb, s, ks, y0, tid, tbase, false, nx, gs.mu, gs.sigma_mol, rv, kn);
             if (live) sa.out[row + k] = d;
             __syncthreads();
             continue;
@@ -558,8 +649,10 @@ coag_cells_kernel(const DevTables tb, const GasArgs gs, const StepArgs sa_in)
                 ys = yn;
             }
             const bool pre = MODE == MODE_STEP && st == 3 && cell + (int)gridDim.x < sa.C;
-            const double d = eval_rates<NT, SLAB>(tb, s, ks, ys, tid, tbase, pre, nx, gs.mu,
-                                                  gs.sigma_mol, rv);
+            const double *kn = (MODE == MODE_STEPK && st == 3 && cell + (int)gridDim.x < sa.C)
+                                   ? sa.Kin + (size_t)(cell + gridDim.x) * 2 * P : nullptr;
+            const double d = eval_rates<NT, SLAB, PLANAR>(tb, s, ks, ys, tid, tbase, pre, nx, gs.mu,
+                                                  gs.sigma_mol, rv, kn);
             if (st == 3) rv_valid = pre;
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;
