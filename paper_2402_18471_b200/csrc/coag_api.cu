@@ -25,6 +25,9 @@ namespace {
 constexpr unsigned kBinsMagic = 0xC0A6B125u;
 constexpr unsigned kGridMagic = 0xC0A66D1Du;
 constexpr int kMaxBins = 256;
+// cudisc_coag_kernel on the stencil kernel's build: what the whole prologue of the next cell costs a bin-owning warp, in
+// the units of the build cost model of coag_v3_host.cpp (one row of 32 pairs = 95)
+constexpr double kOwnerCostKernelMode = 1300.0;
 
 thread_local char g_err[512] = "";
 std::atomic<long long> g_launches{0};
@@ -55,6 +58,7 @@ struct cudisc_bins_s {
     void *dev_blob;
     DevTables dt;
     V3Tables v3;            // stencil cell kernel tables (v3.on == 0: not applicable to this grid)
+    V3Tables v3k;           // the same kernel's build alone (cudisc_coag_kernel): run lists with the prologue on the bin owners
 };
 
 struct cudisc_grid_s {
@@ -355,6 +359,12 @@ int upload_tables(cudisc_bins b)
     d.sched = (const int *)(base + o_sc);
     b->dt = d;
     b->v3 = V.t;
+    {
+        V3Host Vk;
+        v3_build(t, d.logGrid, optin, Vk, kOwnerCostKernelMode, true);
+        b->v3k = Vk.t;
+        if (!V.t.on) b->v3k.on = 0;
+    }
     b->dev_blob = blob;
     b->device = dev;
     b->on_device = true;
@@ -410,7 +420,10 @@ int run(cudisc_grid g, int mode, GasArgs ga, StepArgs sa, cudisc_stream stream, 
     sa.kslab = g->kslab;
     LaunchCfg lc{std::min(g->grid_ctas, std::max(1, sa.C)), g->smem_bytes, g->smem_optin};
     cudaError_t e;
-    if (g->fast && (mode == MODE_OTF || mode == MODE_STEP) && !ga.hd && !ga.vphi) {
+    if (g->fast && mode == MODE_KERNEL && g->bins->v3k.on && !ga.hd && !ga.vphi) {
+        LaunchCfg lf{std::min(g->fast_ctas, std::max(1, sa.C)), g->bins->v3k.smemBytes, g->smem_optin};
+        e = launch_v3(mode, lf, g->bins->dt, g->bins->v3k, ga, sa, (cudaStream_t)stream);
+    } else if (g->fast && (mode == MODE_OTF || mode == MODE_STEP) && !ga.hd && !ga.vphi) {
         LaunchCfg lf{std::min(g->fast_ctas, std::max(1, sa.C)), g->bins->v3.smemBytes, g->smem_optin};
         e = launch_v3(mode, lf, g->bins->dt, g->bins->v3, ga, sa, (cudaStream_t)stream);
     } else {
@@ -618,6 +631,15 @@ int cudisc_bins_schedule_check(cudisc_bins b, long long *out)
     V3Host V;
     v3_build(t, d.logGrid, 232448, V);
     if (V.t.on) v3_check(t, V, bad);
+    if (V.t.on) {       // the build-only run lists of cudisc_coag_kernel: every pair built exactly once
+        V3Host Vk;
+        v3_build(t, d.logGrid, 232448, Vk, kOwnerCostKernelMode, true);
+        if (Vk.t.on) {
+            long long bk[6] = {0, 0, 0, 0, 0, 0};
+            v3_check(t, Vk, bk);
+            bad[0] += bk[0];
+        }
+    }
     for (int q = 0; q < 6; ++q) out[q] = bad[q];
     out[6] = (long long)S.buildItems.size() + (long long)S.evalItems.size();
     out[7] = (long long)(smem_vec_doubles(Np, d.partRowSlots, d.partColSlots, d.nBuildItems + d.nEvalItems, d.bandD)

@@ -104,8 +104,11 @@ __device__ __forceinline__ VSm v3_carve(char *base, const DevTables &tb, const V
 // ------------------------------------------------------------------------------------------ build
 // rows [32 c + 8 k0, ...) of column block c in chunks of 8 rows (all rows >= 32 c + 32: no diagonal pair);
 // lanes <-> columns j = 32 c + lane.  Two rows per iteration.
+// KOUT (cudisc_coag_kernel): the pairs go to the planes kout[2][P] in HBM (a warp stores 256 contiguous bytes per
+// row and plane) and nowhere else.
+template <bool KOUT>
 __device__ __forceinline__ void v3_build_rows(const V3Tables &vt, const VSm &f, const PairConst &pc,
-                                              const V3ColRun &run, uint32_t tq, int lane)
+                                              const V3ColRun &run, uint32_t tq, int lane, double *kout = nullptr)
 {
     const Smem &s = f.s;
     const int N = vt.N;
@@ -124,6 +127,12 @@ __device__ __forceinline__ void v3_build_rows(const V3Tables &vt, const VSm &f, 
         const RoleI A2 = load_role_i<false, false>(s, i2);
         const double2 k1 = pair_kernel<false, true, false>(A1, B, i - j, pc, s);
         double2 k2 = pair_kernel<false, true, false>(A2, B, i2 - j, pc, s);
+        if (KOUT) {
+            double *ko = kout + tri(i) + j;
+            __stcs(ko, k1.x); __stcs(ko + vt.P, k1.y);
+            if (two) { __stcs(ko + i + 1, k2.x); __stcs(ko + vt.P + i + 1, k2.y); }
+            continue;
+        }
         kr[0] = k1;
         if (two) kr[i + 1] = k2;
         else k2 = make_double2(0.0, 0.0);            // the row past the grid stays 0 in the column copy
@@ -136,9 +145,11 @@ __device__ __forceinline__ void v3_build_rows(const V3Tables &vt, const VSm &f, 
 }
 
 // diagonal block c: rows folded two to a warp (V3Tables::foldA / foldB), two folded rows per iteration;
-// then the block goes to tensor memory with zeros above the diagonal.
+// then the block goes to tensor memory with zeros above the diagonal.  KOUT: straight to the planes in HBM, diagonal
+// not halved (the planes hold K itself; the calls that read them halve it).
+template <bool KOUT>
 __device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, const PairConst &pc,
-                                              const V3ColRun &run, uint32_t tq, int lane)
+                                              const V3ColRun &run, uint32_t tq, int lane, double *kout = nullptr)
 {
     const Smem &s = f.s;
     const int N = vt.N, c = run.c, nf = f.HOT()->nFold[c];
@@ -162,11 +173,17 @@ __device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, 
         const RoleJ B2 = load_role_j<false>(s, j2);
         double2 k1 = pair_kernel<false, true, true>(A1, B1, i1 - j1, pc, s);
         double2 k2 = pair_kernel<false, true, true>(A2, B2, i2 - j2, pc, s);
+        if (KOUT) {
+            if (ok1) { double *ko = kout + tri(i1) + j1; __stcs(ko, k1.x); __stcs(ko + vt.P, k1.y); }
+            if (ok2) { double *ko = kout + tri(i2) + j2; __stcs(ko, k2.x); __stcs(ko + vt.P, k2.y); }
+            continue;
+        }
         if (i1 == j1) { k1.x *= 0.5; k1.y *= 0.5; }
         if (i2 == j2) { k2.x *= 0.5; k2.y *= 0.5; }
         if (ok1) f.KR[tri(i1) + j1] = k1;
         if (ok2) f.KR[tri(i2) + j2] = k2;
     }
+    if (KOUT) return;
     __syncwarp();
     const int j = 32 * c + lane;
     const int iSj = (j < N) ? ((f.BINI()[j].x >> 9) & 0x1ff) : 0;
@@ -607,6 +624,47 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     ProlState ps = {2.0, 0.0, 0.0, 0.0};
     bool rv_valid = false;
 
+    if (MODE == MODE_KERNEL) {
+        // cudisc_coag_kernel: the build alone, every pair straight to the planes in HBM.  The bin-owning warps also
+        // run the whole prologue of the CTA's next cell (in registers) after their share of the rows -- the host
+        // deals them fewer rows (V3Tables built with buildOnly) --, and store its role vectors between two barriers.
+        rv = prologue_compute(tb, g0, gs.mu, gs.sigma_mol, c2, k);
+        if (warp < nb) prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
+        if (tid == 0) s.RED[95] = rv.Vg2;
+        __syncthreads();
+        for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
+            pc.Vg2 = s.RED[95];
+            const int nxt = cell + (int)gridDim.x;
+            const bool pre = nxt < sa.C && warp < nb;
+            CellGas gn = {1.0, 1.0, 1.0, 1.0};
+            if (pre) {
+                gn.T = __ldg(gs.T + nxt); gn.rho_g = __ldg(gs.rho_g + nxt); gn.Om = __ldg(gs.Omega + nxt);
+                gn.alpha = gs.alpha ? __ldg(gs.alpha + nxt) : gs.alpha_const;
+                fetch_vel(nxt);
+            }
+            double *kout = sa.out + (size_t)cell * 2 * vt.P;
+#pragma unroll 1
+            for (int r = 0; r < kV3ColRuns; ++r) {
+                const uint32_t w = reinterpret_cast<const uint32_t *>(smem_v3 + kV3oRUNS)[8 * warp + r];
+                if (!w) break;
+                const V3ColRun run = v3_unpack_col(w);
+                if (run.diag) v3_build_diag<true>(vt, f, pc, run, tq, lane, kout);
+                else v3_build_rows<true>(vt, f, pc, run, tq, lane, kout);
+            }
+            if (pre) rv = prologue_compute(tb, gn, gs.mu, gs.sigma_mol, c2, k);
+            __syncthreads();                              // the role vectors of this cell are dead
+            if (pre) {
+                prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
+                if (tid == 0) s.RED[95] = rv.Vg2;
+            }
+            __syncthreads();
+        }
+        tmem_fence_before();
+        __syncthreads();
+        if (tid < 32) tmem_dealloc_all(tbase);
+        return;
+    }
+
     int err_cell = -1;          // cell whose warp error maxima wait in RED[64 ..) for the next barrier
     auto flush_err = [&]() {
         if (MODE == MODE_STEP && tid == NT - 32 && err_cell >= 0) {     // (a thread of the warp that owns no bins)
@@ -640,8 +698,8 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             const uint32_t w = reinterpret_cast<const uint32_t *>(smem_v3 + kV3oRUNS)[8 * warp + r];
             if (!w) break;
             const V3ColRun run = v3_unpack_col(w);
-            if (run.diag) v3_build_diag(vt, f, pc, run, tq, lane);
-            else v3_build_rows(vt, f, pc, run, tq, lane);
+            if (run.diag) v3_build_diag<false>(vt, f, pc, run, tq, lane);
+            else v3_build_rows<false>(vt, f, pc, run, tq, lane);
         }
         tmem_wait_st();
         cp_async_wait_all();
@@ -754,6 +812,7 @@ cudaError_t launch_v3(int mode, const LaunchCfg &lc, const DevTables &tb, const 
                       const GasArgs &gs, const StepArgs &sa, cudaStream_t st)
 {
     if (mode == MODE_OTF) return launch_v3_mode<MODE_OTF>(lc, tb, vt, gs, sa, st);
+    if (mode == MODE_KERNEL) return launch_v3_mode<MODE_KERNEL>(lc, tb, vt, gs, sa, st);
     return launch_v3_mode<MODE_STEP>(lc, tb, vt, gs, sa, st);
 }
 

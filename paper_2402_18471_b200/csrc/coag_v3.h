@@ -146,7 +146,11 @@ struct V3Host {
 };
 
 // Builds the stencil, checks it against the gather entries and deals the work out.  smem_optin: device limit.
-void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out);
+// ownerBuildCost >= 0: cost units that the bin-owning warps carry in the build phase besides their rows (default:
+// the late start of the step / rates kernels); buildOnly: tables for cudisc_coag_kernel, whose build writes K to HBM
+// and nothing to tensor memory (no tensor-memory capacity limit; only the build runs of the result are used).
+void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out, double ownerBuildCost = -1.0,
+              bool buildOnly = false);
 
 // Host-side check of the run lists and of the stencil (CPU tests, cudisc_bins_schedule_check): adds to
 //   bad[0] pairs not built exactly once            bad[1] bulk pairs not in the row pass exactly once

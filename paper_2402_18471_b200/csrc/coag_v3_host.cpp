@@ -27,8 +27,11 @@ struct Key {
 
 }  // namespace
 
-void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
+void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out, double ownerBuildCost, bool buildOnly)
 {
+    // what the bin-owning warps carry in the build phase besides their rows: a late start (step / rates kernels: they
+    // assemble and finish the previous cell first) or the whole prologue of the next cell (cudisc_coag_kernel)
+    const double ownerLate = ownerBuildCost >= 0.0 ? ownerBuildCost : kCBuildOwnerLate;
     V3Tables &t = out.t;
     memset(&t, 0, sizeof(t));
     out.why.clear();
@@ -143,7 +146,7 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
     // ------------------------------------------------------------------ column chunks -> warps
     if (3 * nb > kV3Warps) { out.why = "too many bins for the three combine groups"; return; }
     int cap[4];
-    for (int q = 0; q < 4; ++q) cap[q] = 512 / 32;
+    for (int q = 0; q < 4; ++q) cap[q] = buildOnly ? 1 << 20 : 512 / 32;     // (build only: nothing goes to tensor memory)
     // diagonal blocks: folded row pairs
     double diagCost[kV3MaxBlk];
     for (int c = 0; c < nb; ++c) {
@@ -176,14 +179,14 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
             total += kCBuildRow * rows;
         }
     }
-    total += kCBuildOwnerLate * nb;
+    total += ownerLate * nb;
     const double T = total / kV3Warps;
     std::vector<std::vector<Chunk>> mine(kV3Warps);
     double load[kV3Warps] = {0};
     int qfill[4] = {0, 0, 0, 0};
     int diagWarp[kV3MaxBlk];
     // the bin-owning warps join the build late: they assemble and finish the previous cell first (coag_v3.cu)
-    for (int w = 0; w < nb; ++w) load[w] = kCBuildOwnerLate;
+    for (int w = 0; w < nb; ++w) load[w] = ownerLate;
     for (int c = 0; c < nb; ++c) {
         const int w = kV3Warps - 1 - c;                 // away from the bin-owning warps
         diagWarp[c] = w;
@@ -217,7 +220,7 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
         for (int c = 0; c < nb; ++c)
             if (diagWarp[c] == w) {
                 const int n = (std::min(32, N - 32 * c) + 7) / 8;
-                cr[w].push_back({c, 0, n, tcolNext[w & 3], 0, 1});
+                cr[w].push_back({c, 0, n, buildOnly ? 0 : tcolNext[w & 3], 0, 1});
                 tcolNext[w & 3] += 32 * n;
             }
         std::sort(mine[w].begin(), mine[w].end(), [](const Chunk &x, const Chunk &y) {
@@ -227,13 +230,13 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out)
             if (!cr[w].empty() && !cr[w].back().diag && cr[w].back().c == ch.c && cr[w].back().k0 + cr[w].back().n == ch.k)
                 cr[w].back().n++;
             else
-                cr[w].push_back({ch.c, ch.k, 1, tcolNext[w & 3], 0, 0});
+                cr[w].push_back({ch.c, ch.k, 1, buildOnly ? 0 : tcolNext[w & 3], 0, 0});
             tcolNext[w & 3] += 32;
         }
         if ((int)cr[w].size() > kV3ColRuns) { out.why = "too many column runs on a warp"; return; }
     }
     for (int q = 0; q < 4; ++q)
-        if (tcolNext[q] > 512) { out.why = "column copy exceeds tensor memory"; return; }
+        if (!buildOnly && tcolNext[q] > 512) { out.why = "column copy exceeds tensor memory"; return; }
     {
         int slot = 0;
         for (int c = 0; c < nb; ++c) {
