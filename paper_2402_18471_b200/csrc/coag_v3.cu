@@ -202,6 +202,39 @@ __device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, 
     }
 }
 
+// ------------------------------------------------------------------------------------------ K from HBM
+// cudisc_coag_rates / cudisc_coag_step_cached: the row copy is refilled from the planes of a cell in HBM / L2 by 8-byte
+// LDGSTS copies (plane 0 -> .x, plane 1 -> .y of every pair), all threads; completed by cp.async.wait_all + a block
+// barrier.  The column copy is then made from the row copy.
+__device__ __forceinline__ void v3_refill_pairs(double2 *kr, const double *planes, int P, int tid, int nt)
+{
+    for (int p = tid; p < P; p += nt) {
+        cp_async8(&kr[p].x, planes + p);
+        cp_async8(&kr[p].y, planes + P + p);
+    }
+}
+// chunks [k0, k0 + n) of column block c: row copy -> tensor memory (lane <-> column j; zeros above the diagonal and
+// for Kf of rows below iS[j], as the build writes them)
+__device__ __forceinline__ void v3_fill_tmem(const V3Tables &vt, const VSm &f, const V3ColRun &run, uint32_t tq, int lane)
+{
+    const int N = vt.N, c = run.c;
+    const int j = 32 * c + lane;
+    const int iSj = (j < N) ? ((f.BINI()[j].x >> 9) & 0x1ff) : 0;
+#pragma unroll 1
+    for (int kk = 0; kk < run.n; ++kk) {
+        uint32_t v[32];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int i = 32 * c + 8 * (run.k0 + kk) + r;
+            double2 k2 = make_double2(0.0, 0.0);
+            if (i < N && j <= i) k2 = f.KR[tri(i) + j];
+            if (i < iSj) k2.y = 0.0;
+            v[4 * r] = dlo(k2.x); v[4 * r + 1] = dhi(k2.x); v[4 * r + 2] = dlo(k2.y); v[4 * r + 3] = dhi(k2.y);
+        }
+        tmem_st32(tq + (uint32_t)(run.tcol + 32 * kk), v);
+    }
+}
+
 // ------------------------------------------------------------------------------------------ eval pieces
 // column pass of one run: lane <-> impactor column j = 32 c + lane, rows of chunks [k0, k0 + n) from tensor
 // memory; G_j += Kc_ij n_i, H_j += Kf_ij n_i (Kf already 0 where the pair does not count).
@@ -365,7 +398,8 @@ template <int NT>
 __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &vt, const VSm &f, double y,
                                           double c1, double c2, double c3, int tid, uint32_t tq, int ppart,
                                           const CellDerived &nd, const GasArgs &gs, bool deriveNext, ProlState &ps,
-                                          RoleVals &rv, bool storeNext, double nvR, double nvZ)
+                                          RoleVals &rv, bool storeNext, double nvR, double nvZ,
+                                          const double *kin_next = nullptr)
 {
     const int N = vt.N, nb = vt.nb;
     const int lane = tid & 31, warp = tid >> 5;
@@ -415,6 +449,9 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
         v3_row_run(tb, vt, f, v3_unpack_row(w), lane);
     }
     __syncthreads();
+    // (kernel read from HBM, last evaluation of a cell: the row copy is dead from here on, the next cell's planes
+    //  start to arrive under the combine phase)
+    if (kin_next) v3_refill_pairs(f.KR, kin_next, vt.P, tid, NT);
 
     // ---- phase B (combine), three groups of warps side by side:
     //   R (warp w < nb, bin 32 w + lane)      row partials -> deposits into bins k-1, k, k+1; first half of the
@@ -523,7 +560,9 @@ __global__ void __launch_bounds__(NT, 1)
 coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const StepArgs sa_in)
 {
     StepArgs sa = sa_in;
-    if (MODE == MODE_STEP && !apply_ctrl(sa)) return;
+    constexpr bool KIN = MODE == MODE_RATES || MODE == MODE_STEPK;       // the kernel of a cell is read from HBM
+    constexpr bool STEPPING = MODE == MODE_STEP || MODE == MODE_STEPK;   // BS3(2) step (else: one rate evaluation)
+    if (STEPPING && !apply_ctrl(sa)) return;
     extern __shared__ __align__(16) char smem_v3[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
     const int N = vt.N, nb = vt.nb;
@@ -604,16 +643,19 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     };
     // first cell of the CTA: nothing ran ahead, every thread takes the raw values; second cell: its scalars are
     // derived here (once per launch)
-    stage_gas(blockIdx.x);
-    cp_async_wait_all();
-    __syncthreads();
-    const CellGas g0 = raw_gas();
-    fetch_vel(blockIdx.x);
-    __syncthreads();
-    stage_gas(blockIdx.x + gridDim.x);
-    cp_async_wait_all();
-    __syncthreads();
-    if (warp == kV3Warps - 1 && (int)(blockIdx.x + gridDim.x) < sa.C) {
+    CellGas g0 = {1.0, 1.0, 1.0, 1.0};
+    if (!KIN) {
+        stage_gas(blockIdx.x);
+        cp_async_wait_all();
+        __syncthreads();
+        g0 = raw_gas();
+        fetch_vel(blockIdx.x);
+        __syncthreads();
+        stage_gas(blockIdx.x + gridDim.x);
+        cp_async_wait_all();
+        __syncthreads();
+    }
+    if (!KIN && warp == kV3Warps - 1 && (int)(blockIdx.x + gridDim.x) < sa.C) {
         const CellDerived d = derive_cell(raw_gas(), gs.mu, gs.sigma_mol);
         if (lane == 0) {
             s.RED[84] = d.Ste; s.RED[85] = d.den; s.RED[86] = d.Om; s.RED[87] = d.Vg2; s.RED[88] = d.bmc;
@@ -667,7 +709,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
 
     int err_cell = -1;          // cell whose warp error maxima wait in RED[64 ..) for the next barrier
     auto flush_err = [&]() {
-        if (MODE == MODE_STEP && tid == NT - 32 && err_cell >= 0) {     // (a thread of the warp that owns no bins)
+        if (STEPPING && tid == NT - 32 && err_cell >= 0) {     // (a thread of the warp that owns no bins)
             unsigned long long m = 0ull;
 #pragma unroll 1
             for (int w = 0; w < nb; ++w) {
@@ -679,7 +721,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     };
     for (int cell = blockIdx.x; cell < sa.C; cell += gridDim.x) {
         const size_t row = (size_t)cell * N;
-        if (!rv_valid) {                              // first cell of the CTA: nothing ran ahead
+        if (!KIN && !rv_valid) {                      // first cell of the CTA: nothing ran ahead
             rv = prologue_compute(tb, g0, gs.mu, gs.sigma_mol, c2, k);
             prologue_store(tb, rv, nvR, nvZ, 0.0, false, false, s, k);
             if (tid == 0) s.RED[95] = rv.Vg2;
@@ -690,15 +732,39 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         // copies into (y, y m) -- free during the build -- and RED, landed by the post-build barrier
         if (live) {
             cp_async8(&f.YY()[k].x, sa.rho + row + k);
-            if (MODE == MODE_STEP && sa.have_k1) cp_async8(&f.YY()[k].y, sa.k_fsal + row + k);
+            if (STEPPING && sa.have_k1) cp_async8(&f.YY()[k].y, sa.k_fsal + row + k);
         }
-        stage_gas(cell + 2 * gridDim.x);
+        if (!KIN) stage_gas(cell + 2 * gridDim.x);
+        if (KIN) {
+            // the planes of this cell: on their way since the last evaluation of the CTA's previous cell (v3_eval);
+            // then the diagonal is halved in place and every warp copies its chunks to tensor memory
+            if (cell == (int)blockIdx.x) v3_refill_pairs(f.KR, sa.Kin + (size_t)cell * 2 * vt.P, vt.P, tid, NT);
+            cp_async_wait_all();
+            __syncthreads();
+            if (live) {
+                double2 *dg = f.KR + tri(k) + k;
+                const double2 v = *dg;
+                *dg = make_double2(0.5 * v.x, 0.5 * v.y);
+            }
+            __syncthreads();
+            // while this cell is evaluated its successor's planes are pulled into L2 (asynchronous bulk prefetch)
+            if (cell + (int)gridDim.x < sa.C && (reinterpret_cast<uintptr_t>(sa.Kin) & 15) == 0) {
+                const char *nxt = reinterpret_cast<const char *>(sa.Kin + (size_t)(cell + gridDim.x) * 2 * vt.P);
+                const size_t bytes = 16 * (size_t)vt.P;
+                constexpr size_t kChunk = 8192;
+                for (size_t off = (size_t)tid * kChunk; off < bytes; off += (size_t)NT * kChunk) {
+                    const uint32_t n = (uint32_t)(bytes - off < kChunk ? bytes - off : kChunk);
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(nxt + off), "r"(n) : "memory");
+                }
+            }
+        }
 #pragma unroll 1
         for (int r = 0; r < kV3ColRuns; ++r) {
             const uint32_t w = reinterpret_cast<const uint32_t *>(smem_v3 + kV3oRUNS)[8 * warp + r];
             if (!w) break;
             const V3ColRun run = v3_unpack_col(w);
-            if (run.diag) v3_build_diag<false>(vt, f, pc, run, tq, lane);
+            if (KIN) v3_fill_tmem(vt, f, run, tq, lane);
+            else if (run.diag) v3_build_diag<false>(vt, f, pc, run, tq, lane);
             else v3_build_rows<false>(vt, f, pc, run, tq, lane);
         }
         tmem_wait_st();
@@ -706,9 +772,9 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         double y0 = 0.0, k1 = 0.0;
         if (live) {                                   // the thread's own copies are complete
             y0 = f.YY()[k].x;
-            if (MODE == MODE_STEP && sa.have_k1) k1 = f.YY()[k].y;
+            if (STEPPING && sa.have_k1) k1 = f.YY()[k].y;
         }
-        if (MODE == MODE_STEP && warp < nb) {
+        if (STEPPING && warp < nb) {
             double ws = y0;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
@@ -717,7 +783,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         tmem_fence_before();
         __syncthreads();
         tmem_fence_after();
-        take_derived();
+        if (!KIN) take_derived();
         flush_err();
         // the role vectors are dead: zero the padding of the band stage (its bins are written per evaluation)
         {   // (16 threads per stage row; the host checks that this covers them)
@@ -726,6 +792,13 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         }
 
         const bool more = cell + (int)gridDim.x < sa.C, more2 = cell + 2 * (int)gridDim.x < sa.C;
+        const double *kin_next = (KIN && more) ? sa.Kin + (size_t)(cell + gridDim.x) * 2 * vt.P : nullptr;
+        if (MODE == MODE_RATES) {
+            const double d = v3_eval<NT>(tb, vt, f, y0, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv, false, nvR, nvZ,
+                                         kin_next);
+            if (live) sa.out[row + k] = d;
+            continue;
+        }
         if (MODE == MODE_OTF) {
             fetch_vel(cell + gridDim.x);
             const double d = v3_eval<NT>(tb, vt, f, y0, c1, c2, c3, tid, tq, more ? 4 : 0, nd, gs, more2, ps, rv,
@@ -743,13 +816,15 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             double ys = y0;
             if (st == 1) ys = y0 + 0.5 * h * k1;
             if (st == 2) ys = y0 + 0.75 * h * k2;
-            if (st == 2) fetch_vel(cell + gridDim.x);
+            if (!KIN && st == 2) fetch_vel(cell + gridDim.x);
             if (st == 3) {
                 yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
                 ys = yn;
             }
-            const double d = v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nd, gs, more2 && st == 1,
-                                         ps, rv, more && st == 3, nvR, nvZ);
+            const double d = KIN ? v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv, false, nvR,
+                                               nvZ, st == 3 ? kin_next : nullptr)
+                                 : v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nd, gs,
+                                               more2 && st == 1, ps, rv, more && st == 3, nvR, nvZ);
             if (st == 3) rv_valid = more;
             if (st == 0) k1 = d;
             if (st == 1) k2 = d;
@@ -813,6 +888,8 @@ cudaError_t launch_v3(int mode, const LaunchCfg &lc, const DevTables &tb, const 
 {
     if (mode == MODE_OTF) return launch_v3_mode<MODE_OTF>(lc, tb, vt, gs, sa, st);
     if (mode == MODE_KERNEL) return launch_v3_mode<MODE_KERNEL>(lc, tb, vt, gs, sa, st);
+    if (mode == MODE_RATES) return launch_v3_mode<MODE_RATES>(lc, tb, vt, gs, sa, st);
+    if (mode == MODE_STEPK) return launch_v3_mode<MODE_STEPK>(lc, tb, vt, gs, sa, st);
     return launch_v3_mode<MODE_STEP>(lc, tb, vt, gs, sa, st);
 }
 
