@@ -423,9 +423,8 @@ int run(cudisc_grid g, int mode, GasArgs ga, StepArgs sa, cudisc_stream stream, 
     if (g->fast && mode == MODE_KERNEL && g->bins->v3k.on && !ga.hd && !ga.vphi) {
         LaunchCfg lf{std::min(g->fast_ctas, std::max(1, sa.C)), g->bins->v3k.smemBytes, g->smem_optin};
         e = launch_v3(mode, lf, g->bins->dt, g->bins->v3k, ga, sa, (cudaStream_t)stream);
-    } else if (g->fast && (mode == MODE_OTF || mode == MODE_STEP || mode == MODE_STEPK) && !ga.hd && !ga.vphi) {
-        // (cudisc_coag_rates stays on the general kernel: one evaluation per load, and its TMA refill of a planar store
-        //  beats the stencil kernel's LDGSTS refill of pairs -- 0.99 against 1.05 ms on 16000 cells x 150 bins)
+    } else if (g->fast && (mode == MODE_OTF || mode == MODE_STEP || mode == MODE_RATES || mode == MODE_STEPK) && !ga.hd &&
+               !ga.vphi) {
         LaunchCfg lf{std::min(g->fast_ctas, std::max(1, sa.C)), g->bins->v3.smemBytes, g->smem_optin};
         e = launch_v3(mode, lf, g->bins->dt, g->bins->v3, ga, sa, (cudaStream_t)stream);
     } else {

@@ -93,28 +93,6 @@ __device__ __forceinline__ void build_cell(const DevTables &tb, const Smem &s, c
 // ------------------------------------------------------------------------------------------ eval
 // One rate evaluation of the current cell: thread k < N passes y_k and gets drho_k/dt.
 // Three block barriers; every partial sum has its own slot and every combination a fixed order.
-// Asynchronous refill of a PLANAR K store from the planes of a cell: 1-D bulk copies (TMA) of the 16 P bytes,
-// completing on an mbarrier.  Called by one thread, after a block barrier behind the last read of the old contents.
-__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void refill_bulk(void *ksm, const double *planes, int P, uint64_t *bar)
-{
-    const uint32_t bytes = 16u * (uint32_t)P;
-    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" :: "r"(smem_addr(bar)), "r"(bytes) : "memory");
-    constexpr uint32_t kChunk = 32768;
-    for (uint32_t off = 0; off < bytes; off += kChunk) {
-        const uint32_t n = bytes - off < kChunk ? bytes - off : kChunk;
-        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                     :: "r"(smem_addr(ksm) + off), "l"(reinterpret_cast<const char *>(planes) + off), "r"(n),
-                        "r"(smem_addr(bar)) : "memory");
-    }
-}
-__device__ __forceinline__ void mbar_wait_parity(uint64_t *bar, uint32_t parity)
-{
-    asm volatile("{\n.reg .pred p;\nWAIT_%=:\n"
-                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-                 "@!p bra WAIT_%=;\n}\n" :: "r"(smem_addr(bar)), "r"(parity) : "memory");
-}
 constexpr int kRedMbar = 88;     // Smem::RED slot that holds the mbarrier of the refill
 
 // The same for a store of (Kc, Kf) pairs (cudisc_coag_step_cached: three evaluations per load, and the pair layout

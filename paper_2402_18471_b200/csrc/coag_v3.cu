@@ -80,6 +80,18 @@ struct VSm {
     __device__ __forceinline__ const V3Hot *HOT() const { return reinterpret_cast<const V3Hot *>(base + kV3oHOT); }
 };
 
+// a pair of the row copy: (Kc, Kf) pairs at KR[p], or -- PLANAR, cudisc_coag_rates: the store is the image of a cell's
+// planes in HBM, filled by bulk copies -- two doubles P apart
+template <bool PLANAR>
+__device__ __forceinline__ double2 v3_kld(const double2 *KR, int P, int p)
+{
+    if (PLANAR) {
+        const double *d = reinterpret_cast<const double *>(KR);
+        return make_double2(d[p], d[P + p]);
+    }
+    return KR[p];
+}
+
 __device__ __forceinline__ VSm v3_carve(char *base, const DevTables &tb, const V3Tables &vt)
 {
     VSm f;
@@ -203,18 +215,13 @@ __device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, 
 }
 
 // ------------------------------------------------------------------------------------------ K from HBM
-// cudisc_coag_rates / cudisc_coag_step_cached: the row copy is refilled from the planes of a cell in HBM / L2 by 8-byte
-// LDGSTS copies (plane 0 -> .x, plane 1 -> .y of every pair), all threads; completed by cp.async.wait_all + a block
-// barrier.  The column copy is then made from the row copy.
-__device__ __forceinline__ void v3_refill_pairs(double2 *kr, const double *planes, int P, int tid, int nt)
-{
-    for (int p = tid; p < P; p += nt) {
-        cp_async8(&kr[p].x, planes + p);
-        cp_async8(&kr[p].y, planes + P + p);
-    }
-}
+// cudisc_coag_rates / cudisc_coag_step_cached: the row copy is the image of a cell's planes in HBM ([2][P] doubles,
+// PLANAR), refilled by 1-D bulk copies (TMA, refill_bulk of coag_device.cuh) that complete on an mbarrier in RED; the
+// column copy is then made from the row copy.
+constexpr int kV3RedMbar = 90;
 // chunks [k0, k0 + n) of column block c: row copy -> tensor memory (lane <-> column j; zeros above the diagonal and
 // for Kf of rows below iS[j], as the build writes them)
+template <bool PLANAR>
 __device__ __forceinline__ void v3_fill_tmem(const V3Tables &vt, const VSm &f, const V3ColRun &run, uint32_t tq, int lane)
 {
     const int N = vt.N, c = run.c;
@@ -227,7 +234,7 @@ __device__ __forceinline__ void v3_fill_tmem(const V3Tables &vt, const VSm &f, c
         for (int r = 0; r < 8; ++r) {
             const int i = 32 * c + 8 * (run.k0 + kk) + r;
             double2 k2 = make_double2(0.0, 0.0);
-            if (i < N && j <= i) k2 = f.KR[tri(i) + j];
+            if (i < N && j <= i) k2 = v3_kld<PLANAR>(f.KR, vt.P, tri(i) + j);
             if (i < iSj) k2.y = 0.0;
             v[4 * r] = dlo(k2.x); v[4 * r + 1] = dhi(k2.x); v[4 * r + 2] = dlo(k2.y); v[4 * r + 3] = dhi(k2.y);
         }
@@ -270,6 +277,7 @@ __device__ __forceinline__ void v3_col_run(const V3Tables &vt, const VSm &f, con
 // row pass of one run: lane <-> target row i = 32 b + lane, impactor columns [ja, jb) clipped to the bulk
 // prefix j < n_bulk[i]:  A1, A2 += Kc_ij (y_j, y_j m_j);  F1, F2 += Kf_ij (y_j, y_j m_j).  The slot takes
 // the deposits per unit n_i into bins i - 1, i, i + 1 (coefficients of coag_tables.h, read through L1).
+template <bool PLANAR>
 __device__ __forceinline__ void v3_row_run(const DevTables &tb, const V3Tables &vt, const VSm &f, const V3RowRun &run,
                                            int lane)
 {
@@ -280,7 +288,8 @@ __device__ __forceinline__ void v3_row_run(const DevTables &tb, const V3Tables &
     const int Nq = tb.Np;
     const double cA1 = __ldg(bc + BC_A1 * Nq), cA2 = __ldg(bc + BC_A2 * Nq), cB1 = __ldg(bc + BC_B1 * Nq);
     const double cF1 = __ldg(bc + BC_F1 * Nq), cF2 = __ldg(bc + BC_F2 * Nq), cG1 = __ldg(bc + BC_G1 * Nq);
-    const double2 *kr = f.KR + tri(iv);
+    const double2 *kr = f.KR + tri(iv);                              // (pairs)
+    const double *kc = reinterpret_cast<const double *>(f.KR) + tri(iv), *kf = kc + vt.P;     // (PLANAR)
     const double2 *yy = f.YY();
     double a1 = 0.0, a2 = 0.0, f1 = 0.0, f2 = 0.0, b1 = 0.0, b2 = 0.0, g1 = 0.0, g2 = 0.0;
     int j = run.ja;
@@ -288,7 +297,8 @@ __device__ __forceinline__ void v3_row_run(const DevTables &tb, const V3Tables &
     // the rectangle: every row of the block has these columns
 #pragma unroll 4
     for (; j + 2 <= jr; j += 2) {
-        const double2 k2 = kr[j], k3 = kr[j + 1];
+        const double2 k2 = PLANAR ? make_double2(kc[j], kf[j]) : kr[j];
+        const double2 k3 = PLANAR ? make_double2(kc[j + 1], kf[j + 1]) : kr[j + 1];
         const double2 y2 = yy[j], y3 = yy[j + 1];
         a1 = fma(k2.x, y2.x, a1); a2 = fma(k2.x, y2.y, a2);
         f1 = fma(k2.y, y2.x, f1); f2 = fma(k2.y, y2.y, f2);
@@ -299,7 +309,7 @@ __device__ __forceinline__ void v3_row_run(const DevTables &tb, const V3Tables &
     // unconditional -- past the end of a row they hit the next rows of the packed array
 #pragma unroll 4
     for (; j < run.jb; ++j) {
-        const double2 k2 = kr[j];
+        const double2 k2 = PLANAR ? make_double2(kc[j], kf[j]) : kr[j];
         double2 y2 = yy[j];
         const bool on = j < nbi;                     // (selects, not branches: the warp stays converged)
         y2.x = on ? y2.x : 0.0; y2.y = on ? y2.y : 0.0;
@@ -315,11 +325,12 @@ __device__ __forceinline__ void v3_row_run(const DevTables &tb, const V3Tables &
 
 // band stage of the bins 32 g + lane (coag_v3.h): W[plane][d][i] = y_i n_{i-d} Kplane[i][i-d], 0 where the
 // pair does not exist; yi: the thread's own y (0 for i >= N)
+template <bool PLANAR>
 __device__ __forceinline__ void v3_stage(const V3Tables &vt, const VSm &f, int i, double yi)
 {
     const int N = vt.N, D = vt.bandD;
     const int iv = min(i, N - 1);
-    const double2 *kr = f.KR + tri(iv) + iv;
+    const int pd = tri(iv) + iv;                     // the diagonal pair of row iv
     const double *nn = f.NN() + iv;
     double *w = f.WST() + vt.wPad + i;
     const int plane = D * vt.wRow;
@@ -327,7 +338,7 @@ __device__ __forceinline__ void v3_stage(const V3Tables &vt, const VSm &f, int i
     for (int d = 0; d < D; ++d) {
         double wc = 0.0, wf = 0.0;
         if (d <= iv) {
-            const double2 k2 = kr[-d];
+            const double2 k2 = v3_kld<PLANAR>(f.KR, vt.P, pd - d);
             const double yn = yi * nn[-d];
             wc = yn * k2.x; wf = yn * k2.y;
         }
@@ -394,7 +405,7 @@ __device__ __forceinline__ double v3_staps(const V3Tables &vt, const VSm &f, con
 // ------------------------------------------------------------------------------------------ eval
 // One rate evaluation: thread k < N passes y_k and gets drho_k/dt.  c1, c2, c3: per-thread constants of the
 // thread's role -- bin owners (warp < nb): m_k, 1 / m_k, A_k; column-combine group (warp nb + g): -, -, 1 / B_k.
-template <int NT>
+template <int NT, bool PLANAR = false>
 __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &vt, const VSm &f, double y,
                                           double c1, double c2, double c3, int tid, uint32_t tq, int ppart,
                                           const CellDerived &nd, const GasArgs &gs, bool deriveNext, ProlState &ps,
@@ -420,7 +431,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
     //      (ppart 1, 2, 3; 4: all of it); then every warp its own runs
     double excA = 0.0;          // density exceptions of the thread's own bin, summed in phase A when they are local
     if (warp < nb) {
-        v3_stage(vt, f, k, live ? y : 0.0);
+        v3_stage<PLANAR>(vt, f, k, live ? y : 0.0);
         if (vt.excLocal) {
             __syncwarp();
             excA = v3_exceptions(f, f.WST(), warp, 0, lane, 0.0);
@@ -446,12 +457,13 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
     for (int r = 0; r < kV3RowRuns; ++r) {
         const uint32_t w = r == 0 ? roww.x : (r == 1 ? roww.y : roww.z);
         if (!w) break;
-        v3_row_run(tb, vt, f, v3_unpack_row(w), lane);
+        v3_row_run<PLANAR>(tb, vt, f, v3_unpack_row(w), lane);
     }
     __syncthreads();
     // (kernel read from HBM, last evaluation of a cell: the row copy is dead from here on, the next cell's planes
     //  start to arrive under the combine phase)
-    if (kin_next) v3_refill_pairs(f.KR, kin_next, vt.P, tid, NT);
+    if (PLANAR && kin_next && tid == 0)
+        refill_bulk(f.KR, kin_next, vt.P, reinterpret_cast<uint64_t *>(f.RED() + kV3RedMbar));
 
     // ---- phase B (combine), three groups of warps side by side:
     //   R (warp w < nb, bin 32 w + lane)      row partials -> deposits into bins k-1, k, k+1; first half of the
@@ -562,6 +574,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     StepArgs sa = sa_in;
     constexpr bool KIN = MODE == MODE_RATES || MODE == MODE_STEPK;       // the kernel of a cell is read from HBM
     constexpr bool STEPPING = MODE == MODE_STEP || MODE == MODE_STEPK;   // BS3(2) step (else: one rate evaluation)
+    constexpr bool PLANAR = KIN;         // row copy = image of the planes in HBM, refilled by bulk copies
     if (STEPPING && !apply_ctrl(sa)) return;
     extern __shared__ __align__(16) char smem_v3[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
@@ -599,6 +612,13 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         c3 = tb.binc[BC_FIB * tb.Np + tid - 32 * nb];
     }
 
+    uint64_t *kbar = reinterpret_cast<uint64_t *>(f.RED() + kV3RedMbar);
+    uint32_t kph = 0u;
+    const bool kin_tma = PLANAR && (reinterpret_cast<uintptr_t>(sa.Kin) & 15) == 0;
+    if (PLANAR && tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" :: "r"(smem_addr(kbar)), "r"(1) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
     uint32_t *slot = reinterpret_cast<uint32_t *>(f.RED());
     if (tid < 32) tmem_alloc_all(slot);
     tmem_fence_before();
@@ -736,15 +756,23 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         }
         if (!KIN) stage_gas(cell + 2 * gridDim.x);
         if (KIN) {
-            // the planes of this cell: on their way since the last evaluation of the CTA's previous cell (v3_eval);
-            // then the diagonal is halved in place and every warp copies its chunks to tensor memory
-            if (cell == (int)blockIdx.x) v3_refill_pairs(f.KR, sa.Kin + (size_t)cell * 2 * vt.P, vt.P, tid, NT);
+            // the planes of this cell: bulk copies on their way since the last evaluation of the CTA's previous cell
+            // (v3_eval: behind the last read of the row copy, under the combine phase); then the diagonal is halved
+            // in place and every warp copies its chunks to tensor memory
+            const double *planes = sa.Kin + (size_t)cell * 2 * vt.P;
+            if (kin_tma) {
+                if (cell == (int)blockIdx.x && tid == 0) refill_bulk(f.KR, planes, vt.P, kbar);
+                mbar_wait_parity(kbar, kph);
+                kph ^= 1u;
+            } else {                                      // planes not 16-byte aligned: plain copy
+                double *img = reinterpret_cast<double *>(f.KR);
+                for (int p = tid; p < 2 * vt.P; p += NT) img[p] = __ldcs(planes + p);
+            }
             cp_async_wait_all();
             __syncthreads();
             if (live) {
-                double2 *dg = f.KR + tri(k) + k;
-                const double2 v = *dg;
-                *dg = make_double2(0.5 * v.x, 0.5 * v.y);
+                double *img = reinterpret_cast<double *>(f.KR) + tri(k) + k;
+                img[0] *= 0.5; img[vt.P] *= 0.5;
             }
             __syncthreads();
             // while this cell is evaluated its successor's planes are pulled into L2 (asynchronous bulk prefetch)
@@ -763,7 +791,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             const uint32_t w = reinterpret_cast<const uint32_t *>(smem_v3 + kV3oRUNS)[8 * warp + r];
             if (!w) break;
             const V3ColRun run = v3_unpack_col(w);
-            if (KIN) v3_fill_tmem(vt, f, run, tq, lane);
+            if (KIN) v3_fill_tmem<PLANAR>(vt, f, run, tq, lane);
             else if (run.diag) v3_build_diag<false>(vt, f, pc, run, tq, lane);
             else v3_build_rows<false>(vt, f, pc, run, tq, lane);
         }
@@ -792,9 +820,9 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         }
 
         const bool more = cell + (int)gridDim.x < sa.C, more2 = cell + 2 * (int)gridDim.x < sa.C;
-        const double *kin_next = (KIN && more) ? sa.Kin + (size_t)(cell + gridDim.x) * 2 * vt.P : nullptr;
+        const double *kin_next = (KIN && more && kin_tma) ? sa.Kin + (size_t)(cell + gridDim.x) * 2 * vt.P : nullptr;
         if (MODE == MODE_RATES) {
-            const double d = v3_eval<NT>(tb, vt, f, y0, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv, false, nvR, nvZ,
+            const double d = v3_eval<NT, PLANAR>(tb, vt, f, y0, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv, false, nvR, nvZ,
                                          kin_next);
             if (live) sa.out[row + k] = d;
             continue;
@@ -821,7 +849,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
                 yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
                 ys = yn;
             }
-            const double d = KIN ? v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv, false, nvR,
+            const double d = KIN ? v3_eval<NT, PLANAR>(tb, vt, f, ys, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv, false, nvR,
                                                nvZ, st == 3 ? kin_next : nullptr)
                                  : v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nd, gs,
                                                more2 && st == 1, ps, rv, more && st == 3, nvR, nvZ);
