@@ -221,12 +221,13 @@ __device__ __forceinline__ void v3_build_diag(const V3Tables &vt, const VSm &f, 
 constexpr int kV3RedMbar = 90;
 // chunks [k0, k0 + n) of column block c: row copy -> tensor memory (lane <-> column j; zeros above the diagonal and
 // for Kf of rows below iS[j], as the build writes them)
-template <bool PLANAR>
+template <bool PLANAR, bool ONFLY>
 __device__ __forceinline__ void v3_fill_tmem(const V3Tables &vt, const VSm &f, const V3ColRun &run, uint32_t tq, int lane)
 {
     const int N = vt.N, c = run.c;
     const int j = 32 * c + lane;
     const int iSj = (j < N) ? ((f.BINI()[j].x >> 9) & 0x1ff) : 0;
+    const bool halve = ONFLY && run.diag && !vt.diagBulk;     // (only a diagonal block holds diagonal pairs)
 #pragma unroll 1
     for (int kk = 0; kk < run.n; ++kk) {
         uint32_t v[32];
@@ -235,6 +236,7 @@ __device__ __forceinline__ void v3_fill_tmem(const V3Tables &vt, const VSm &f, c
             const int i = 32 * c + 8 * (run.k0 + kk) + r;
             double2 k2 = make_double2(0.0, 0.0);
             if (i < N && j <= i) k2 = v3_kld<PLANAR>(f.KR, vt.P, tri(i) + j);
+            if (halve && i == j) { k2.x *= 0.5; k2.y *= 0.5; }           // PAPER.md:436 (the planes hold K itself)
             if (i < iSj) k2.y = 0.0;
             v[4 * r] = dlo(k2.x); v[4 * r + 1] = dhi(k2.x); v[4 * r + 2] = dlo(k2.y); v[4 * r + 3] = dhi(k2.y);
         }
@@ -325,7 +327,7 @@ __device__ __forceinline__ void v3_row_run(const DevTables &tb, const V3Tables &
 
 // band stage of the bins 32 g + lane (coag_v3.h): W[plane][d][i] = y_i n_{i-d} Kplane[i][i-d], 0 where the
 // pair does not exist; yi: the thread's own y (0 for i >= N)
-template <bool PLANAR>
+template <bool PLANAR, bool ONFLY>
 __device__ __forceinline__ void v3_stage(const V3Tables &vt, const VSm &f, int i, double yi)
 {
     const int N = vt.N, D = vt.bandD;
@@ -339,7 +341,9 @@ __device__ __forceinline__ void v3_stage(const V3Tables &vt, const VSm &f, int i
         double wc = 0.0, wf = 0.0;
         if (d <= iv) {
             const double2 k2 = v3_kld<PLANAR>(f.KR, vt.P, pd - d);
-            const double yn = yi * nn[-d];
+            // (PLANAR: the store holds K itself; the half of the diagonal pair, is taken here and in
+            //  v3_fill_tmem -- unless the row pass reads diagonal pairs too, vt.diagBulk: then the store was halved)
+            const double yn = (ONFLY && !vt.diagBulk && d == 0 ? 0.5 * yi : yi) * nn[-d];
             wc = yn * k2.x; wf = yn * k2.y;
         }
         if (i < N) {                                 // (rows of the stage hold the N bins + padding)
@@ -405,7 +409,7 @@ __device__ __forceinline__ double v3_staps(const V3Tables &vt, const VSm &f, con
 // ------------------------------------------------------------------------------------------ eval
 // One rate evaluation: thread k < N passes y_k and gets drho_k/dt.  c1, c2, c3: per-thread constants of the
 // thread's role -- bin owners (warp < nb): m_k, 1 / m_k, A_k; column-combine group (warp nb + g): -, -, 1 / B_k.
-template <int NT, bool PLANAR = false>
+template <int NT, bool PLANAR = false, bool ONFLY = false>
 __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &vt, const VSm &f, double y,
                                           double c1, double c2, double c3, int tid, uint32_t tq, int ppart,
                                           const CellDerived &nd, const GasArgs &gs, bool deriveNext, ProlState &ps,
@@ -431,7 +435,7 @@ __device__ __forceinline__ double v3_eval(const DevTables &tb, const V3Tables &v
     //      (ppart 1, 2, 3; 4: all of it); then every warp its own runs
     double excA = 0.0;          // density exceptions of the thread's own bin, summed in phase A when they are local
     if (warp < nb) {
-        v3_stage<PLANAR>(vt, f, k, live ? y : 0.0);
+        v3_stage<PLANAR, ONFLY>(vt, f, k, live ? y : 0.0);
         if (vt.excLocal) {
             __syncwarp();
             excA = v3_exceptions(f, f.WST(), warp, 0, lane, 0.0);
@@ -575,6 +579,10 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
     constexpr bool KIN = MODE == MODE_RATES || MODE == MODE_STEPK;       // the kernel of a cell is read from HBM
     constexpr bool STEPPING = MODE == MODE_STEP || MODE == MODE_STEPK;   // BS3(2) step (else: one rate evaluation)
     constexpr bool PLANAR = KIN;         // row copy = image of the planes in HBM, refilled by bulk copies
+    // The half of the diagonal pairs (the planes hold K itself): taken on the fly by the two readers of
+    // diagonal pairs (band stage, tensor-memory fill) in the step, which saves two block barriers per cell; in place
+    // for the single evaluation of cudisc_coag_rates, where that measured 4 % faster (0.75 against 0.78 ms).
+    constexpr bool ONFLY = MODE == MODE_STEPK;
     if (STEPPING && !apply_ctrl(sa)) return;
     extern __shared__ __align__(16) char smem_v3[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quarter = warp & 3;
@@ -757,8 +765,8 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         if (!KIN) stage_gas(cell + 2 * gridDim.x);
         if (KIN) {
             // the planes of this cell: bulk copies on their way since the last evaluation of the CTA's previous cell
-            // (v3_eval: behind the last read of the row copy, under the combine phase); then the diagonal is halved
-            // in place and every warp copies its chunks to tensor memory
+            // (v3_eval: behind the last read of the row copy, under the combine phase); every thread waits for them
+            // itself, then every warp copies its chunks to tensor memory
             const double *planes = sa.Kin + (size_t)cell * 2 * vt.P;
             if (kin_tma) {
                 if (cell == (int)blockIdx.x && tid == 0) refill_bulk(f.KR, planes, vt.P, kbar);
@@ -767,14 +775,16 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             } else {                                      // planes not 16-byte aligned: plain copy
                 double *img = reinterpret_cast<double *>(f.KR);
                 for (int p = tid; p < 2 * vt.P; p += NT) img[p] = __ldcs(planes + p);
+                __syncthreads();
             }
-            cp_async_wait_all();
-            __syncthreads();
-            if (live) {
-                double *img = reinterpret_cast<double *>(f.KR) + tri(k) + k;
-                img[0] *= 0.5; img[vt.P] *= 0.5;
+            if (!ONFLY || vt.diagBulk) {                  // (always on grids whose bulk row sums reach the diagonal pair)
+                __syncthreads();
+                if (live) {
+                    double *img = reinterpret_cast<double *>(f.KR) + tri(k) + k;
+                    img[0] *= 0.5; img[vt.P] *= 0.5;
+                }
+                __syncthreads();
             }
-            __syncthreads();
             // while this cell is evaluated its successor's planes are pulled into L2 (asynchronous bulk prefetch)
             if (cell + (int)gridDim.x < sa.C && (reinterpret_cast<uintptr_t>(sa.Kin) & 15) == 0) {
                 const char *nxt = reinterpret_cast<const char *>(sa.Kin + (size_t)(cell + gridDim.x) * 2 * vt.P);
@@ -791,7 +801,7 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
             const uint32_t w = reinterpret_cast<const uint32_t *>(smem_v3 + kV3oRUNS)[8 * warp + r];
             if (!w) break;
             const V3ColRun run = v3_unpack_col(w);
-            if (KIN) v3_fill_tmem<PLANAR>(vt, f, run, tq, lane);
+            if (KIN) v3_fill_tmem<PLANAR, ONFLY>(vt, f, run, tq, lane);
             else if (run.diag) v3_build_diag<false>(vt, f, pc, run, tq, lane);
             else v3_build_rows<false>(vt, f, pc, run, tq, lane);
         }
@@ -822,8 +832,8 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
         const bool more = cell + (int)gridDim.x < sa.C, more2 = cell + 2 * (int)gridDim.x < sa.C;
         const double *kin_next = (KIN && more && kin_tma) ? sa.Kin + (size_t)(cell + gridDim.x) * 2 * vt.P : nullptr;
         if (MODE == MODE_RATES) {
-            const double d = v3_eval<NT, PLANAR>(tb, vt, f, y0, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv, false, nvR, nvZ,
-                                         kin_next);
+            const double d = v3_eval<NT, PLANAR, ONFLY>(tb, vt, f, y0, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv,
+                                                        false, nvR, nvZ, kin_next);
             if (live) sa.out[row + k] = d;
             continue;
         }
@@ -849,8 +859,8 @@ coag_v3_kernel(const DevTables tb, const V3Tables vt, const GasArgs gs, const St
                 yn = y0 + h * ((2.0 / 9.0) * k1 + (1.0 / 3.0) * k2 + (4.0 / 9.0) * k3);
                 ys = yn;
             }
-            const double d = KIN ? v3_eval<NT, PLANAR>(tb, vt, f, ys, c1, c2, c3, tid, tq, 0, nd, gs, false, ps, rv, false, nvR,
-                                               nvZ, st == 3 ? kin_next : nullptr)
+            const double d = KIN ? v3_eval<NT, PLANAR, ONFLY>(tb, vt, f, ys, c1, c2, c3, tid, tq, 0, nd, gs, false, ps,
+                                                              rv, false, nvR, nvZ, st == 3 ? kin_next : nullptr)
                                  : v3_eval<NT>(tb, vt, f, ys, c1, c2, c3, tid, tq, more ? st : 0, nd, gs,
                                                more2 && st == 1, ps, rv, more && st == 3, nvR, nvZ);
             if (st == 3) rv_valid = more;

@@ -129,6 +129,8 @@ struct V3Tables {
     int nTaps, nSTaps, nExc, nExcT;
     int nTapsR;                        // taps [0, nTapsR) go to combine group R, the rest to group D (multiples of 8)
     int nExcS;                         // exception entries of S targets (kind 1)
+    int diagBulk;                      // 1: some row's bulk prefix reaches its diagonal pair (coarse grids), so the row pass
+                                       //    reads diagonal pairs and a PLANAR row copy gets its diagonal halved in place
     int excLocal;                      // 1: every density exception reads stage entries of its target's own 32-bin block, so
                                        //    the warp that staged the block sums them right away (phase A)
     // shared-memory byte offsets laid out by the host (the fixed ones are kV3o*)

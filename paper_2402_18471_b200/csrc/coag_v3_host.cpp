@@ -123,6 +123,9 @@ void v3_build(const HostTables &ht, int logGrid, int smem_optin, V3Host &out, do
         V3Tap z; z.c = 0.0; z.off = t.wPad; z.pad = 0;
         t.hot.taps[t.nTaps++] = z;
     }
+    t.diagBulk = 0;
+    for (int i = 0; i < N; ++i)
+        if (ht.n_bulk[i] > i) t.diagBulk = 1;
     t.nTapsR = (2 * t.nTaps / 5) & ~7;
     t.nExcS = 0; t.excLocal = 1;
     for (int q = 0; q < t.nExc; ++q) {

@@ -243,7 +243,16 @@ def _run_manual(N, C, seed, n_r=None, n_z=None, m_centres=None, m_edges=None, st
     y = rho.clone()
     for _ in range(steps):
         cd.cudisc_coag_step(grid, bins, y, dt, err)
+    # the calls that read the kernel from HBM, fed with the library's own K (coarse grids: the bulk row sums reach
+    # the diagonal pair, whose half the kernel store must carry)
+    drho_k = torch.empty_like(drho)
+    cd.cudisc_coag_rates(grid, bins, K, rho, drho_k)
+    err_k = torch.empty_like(err)
+    y_k = rho.clone()
+    for _ in range(steps):
+        cd.cudisc_coag_step_cached(grid, bins, K, y_k, dt, err_k)
     torch.cuda.synchronize()
+    drho_k = drho_k.cpu().numpy(); y_k = y_k.cpu().numpy()
     K = K.cpu().numpy(); drho = drho.cpu().numpy(); y = y.cpu().numpy(); err = err.cpu().numpy()
     iu = np.tril_indices(N)
     for c in range(C):
@@ -256,10 +265,12 @@ def _run_manual(N, C, seed, n_r=None, n_z=None, m_centres=None, m_edges=None, st
         d, _, _, _ = orc.rates_flux(g, Kc, pf, inp["rho"][c])
         _, gain, loss, _ = orc.rates_flux(g, Kc, 0.5 * np.ones_like(pf), inp["rho"][c])   # split-free scale
         assert_rates_close(drho[c:c + 1], d[None], 2.0 * gain[None], 2.0 * loss[None], what=f"cell {c} rates")
+        assert_rates_close(drho_k[c:c + 1], d[None], 2.0 * gain[None], 2.0 * loss[None], what=f"cell {c} rates from K")
         yr, k1, E = inp["rho"][c].copy(), None, 0.0
         for _ in range(steps):
             yr, k1, E = orc.bs32_step(g, Kc, pf, yr, dt, k1=k1)
         assert_rho_close(y[c:c + 1], yr[None], TOL_RHO_1 * steps, f"cell {c} step")
+        assert_rho_close(y_k[c:c + 1], yr[None], TOL_RHO_1 * steps, f"cell {c} cached step")
         assert abs(err[c] - E) <= 1e-6 * abs(E) + 1e-12
         m0 = inp["rho"][c].sum()
         assert abs(y[c].sum() - m0) <= steps * TOL_MASS * m0
