@@ -492,6 +492,7 @@ def run_entry(args):
     torch.cuda.synchronize()
     sampler.stop()
     sec = statistics.mean(e0.elapsed_time(e1) for e0, e1 in ev) * 1e-3
+    fast = bool(bins.fast_path()[0])          # the mass grid takes the stencil kernel (coag_v3.cu)
     pairs = float(C) * P
     evals = {"kernel": 0, "rates": 1, "step_cached": EVALS_PER_STEP}[args.entry]
     hbm_bytes = 16.0 * pairs + (2 if args.entry == "rates" else 6 if args.entry == "step_cached" else 0) * 8.0 * C * N
@@ -510,7 +511,14 @@ def run_entry(args):
                           "achieved": gbs if bound == "hbm" else 2.0 * alu_instr / sec / 1e12,
                           "peak": hbm_peak if bound == "hbm" else 2.0 * sm_count * FP64_LANES_PER_SM * 1965e6 / 1e12,
                           "unit": "GB/s" if bound == "hbm" else "TFLOP/s",
-                          "frac": hbm_frac if bound == "hbm" else alu_frac, "traffic": None,
+                          "frac": hbm_frac if bound == "hbm" else alu_frac,
+                          # dram__bytes_read.sum + dram__bytes_write.sum of one launch (ncu --set full, profiles/
+                          # r02_kernels.md sections 3 - 5), for the profiled workload (config 4, 16000 cells) only
+                          "traffic": ({"kernel": 2897776856, "rates": 2940610528, "step_cached": 2979018016}[args.entry]
+                                      if (args.config == 4 and C == 16000 and fast) else None),
+                          "kernel": ("cudisc::coag_v3_kernel<512, MODE_%s>"
+                                     % {"kernel": "KERNEL", "rates": "RATES", "step_cached": "STEPK"}[args.entry]
+                                     if fast else "cudisc::coag_cells_kernel<512, MODE, SLAB, false>"),
                           "hbm_gbs": gbs, "hbm_frac": hbm_frac, "alu_frac": alu_frac,
                           "how": f"algorithmic HBM bytes per launch = 16 B x {pairs:.4g} pairs (+ the [C x N] arrays) "
                                  f"= {hbm_bytes:.4g} / mean CUDA-event launch duration {1e3 * sec:.3f} ms; HBM peak "
